@@ -1,0 +1,77 @@
+// fdas_common.cuh -- plan object, error plumbing and small device helpers shared by the
+// kernels of libfdas.so (include/fdas.h is the public boundary).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include "../../include/fdas.h"
+
+struct fdas_plan {
+    int64_t n_samples, n_bins, n_cols;
+    int32_t bin0, n_z, n_t, m, L, step, n_seg, interbin, nset;
+    double  z_max, dz;
+    int32_t max_batch, quad_points;
+    int32_t built;
+    // big FFT split of the packed half-length transform: M = n_samples/2 = R1*R2
+    int32_t M, R1, R2, C1, C2, n_part;
+    size_t  ws_inter_bytes, ws_part_bytes, workspace_bytes;
+    // template bank (device, owned)
+    float2* d_taps;   // [n_t][m]  conj R_z(d_j), fp32
+    float2* d_W;      // [n_t][L]  FFT_L(index-reversed taps)/L, in the register layout of the segment kernel
+    // scratch arena of fdas_search_host (device, owned, lazily allocated)
+    void*   arena;
+    size_t  arena_bytes;
+    uint32_t arena_capacity;
+    int32_t  arena_batch;
+};
+
+void fdas_set_cuda_error(cudaError_t e, const char* where);
+
+#define FDAS_CUDA(call)                                          \
+    do {                                                         \
+        cudaError_t _e = (call);                                 \
+        if (_e != cudaSuccess) {                                 \
+            fdas_set_cuda_error(_e, #call);                      \
+            return FDAS_E_CUDA;                                  \
+        }                                                        \
+    } while (0)
+
+#define FDAS_LAUNCH_CHECK() FDAS_CUDA(cudaGetLastError())
+
+// kernel launchers (one per .cu file); all enqueue on `st` and return an FDAS code
+int fdas_launch_templates(fdas_plan* p, cudaStream_t st);
+int fdas_launch_spectrum(fdas_plan* p, const float* d_series, int n_batch, float2* d_spec,
+                         float* d_meanpow, void* d_ws, cudaStream_t st);
+int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float* d_plane, float thr,
+                          fdas_cand* d_cands, uint32_t* d_counts, uint32_t cap, cudaStream_t st);
+int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const float* h_thr,
+                        fdas_cand* d_cands, uint32_t* d_count, uint32_t cap, cudaStream_t st);
+int fdas_launch_candidates(fdas_plan* p, const float* d_plane, float thr, fdas_cand* d_cands,
+                           uint32_t* d_count, uint32_t cap, cudaStream_t st);
+
+// ------------------------------------------------------------------ device helpers
+__device__ __forceinline__ float2 cmul(float2 a, float2 b)
+{
+    return make_float2(fmaf(a.x, b.x, -a.y * b.y), fmaf(a.x, b.y, a.y * b.x));
+}
+__device__ __forceinline__ float2 cadd(float2 a, float2 b) { return make_float2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ float2 csub(float2 a, float2 b) { return make_float2(a.x - b.x, a.y - b.y); }
+
+// exp(sign * 2 pi i * num / den), num/den exact in fp32 (den a power of two)
+__device__ __forceinline__ float2 twiddle(int num, int den, float sign)
+{
+    float s, c;
+    sincospif(2.0f * (float)num / (float)den, &s, &c);
+    return make_float2(c, sign * s);
+}
+
+// Append one candidate; the slot counter receives the true count (include/fdas.h).
+__device__ __forceinline__ void push_cand(fdas_cand* list, uint32_t* count, uint32_t cap,
+                                          int col, int zi, int nharm, float power)
+{
+    uint32_t slot = atomicAdd(count, 1u);
+    if (slot < cap) {
+        fdas_cand c;
+        c.col = col; c.zi = (int16_t)zi; c.nharm = (int16_t)nharm; c.power = power;
+        list[slot] = c;
+    }
+}
