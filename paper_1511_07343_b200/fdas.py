@@ -1,0 +1,257 @@
+"""Thin ctypes binding of libfdas.so (include/fdas.h): argument marshalling only.
+
+Every step of the path runs in the CUDA kernels of the library; PyTorch is used for
+device memory and streams. There is no CPU fallback: a missing library raises.
+Function names mirror the C ABI (`fdas_plan_create`, `fdas_spectrum`, ...); `Plan`
+is a small convenience wrapper that owns the device buffers.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libfdas.so")
+
+FDAS_OK, FDAS_E_INVALID, FDAS_E_STATE, FDAS_E_WORKSPACE, FDAS_E_CUDA, FDAS_E_NOMEM = 0, -1, -2, -3, -4, -5
+FDAS_OPT_INTERBIN, FDAS_OPT_MAX_BATCH, FDAS_OPT_QUAD_POINTS = 1, 2, 3
+
+CAND_DTYPE = np.dtype([("col", "<i4"), ("zi", "<i2"), ("nharm", "<i2"), ("power", "<f4")])
+assert CAND_DTYPE.itemsize == 12
+
+EXPORTS = ["fdas_set_device", "fdas_plan_create", "fdas_plan_set_option", "fdas_plan_info",
+           "fdas_build_templates", "fdas_get_templates", "fdas_spectrum", "fdas_correlate",
+           "fdas_harmsum", "fdas_candidates", "fdas_search_host", "fdas_threshold",
+           "fdas_plan_destroy", "fdas_strerror"]
+
+
+class FdasInfo(C.Structure):
+    _fields_ = [("n_samples", C.c_int64), ("n_bins", C.c_int64), ("n_cols", C.c_int64),
+                ("bin0", C.c_int32), ("n_z", C.c_int32), ("n_templates", C.c_int32), ("width", C.c_int32),
+                ("seg_len", C.c_int32), ("step", C.c_int32), ("n_seg", C.c_int32), ("interbin", C.c_int32),
+                ("z_max", C.c_double), ("dz", C.c_double), ("workspace_bytes", C.c_size_t)]
+
+
+class FdasError(RuntimeError):
+    def __init__(self, code, where):
+        self.code = code
+        super().__init__("%s failed: %d (%s)" % (where, code, lib().fdas_strerror(code).decode()))
+
+
+_lib = None
+
+
+def lib():
+    """Load libfdas.so (raises if it has not been built: there is no fallback path)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("libfdas.so not built: run `python -m paper_1511_07343_b200.build` "
+                              "(or __graft_entry__.build()); the CUDA library is required")
+        L = C.CDLL(LIB_PATH)
+        vp, i32, i64, u32, f32, f64 = C.c_void_p, C.c_int32, C.c_int64, C.c_uint32, C.c_float, C.c_double
+        L.fdas_set_device.argtypes = [i32]
+        L.fdas_plan_create.argtypes = [C.POINTER(vp), i64, f64, f64, i32, i32]
+        L.fdas_plan_set_option.argtypes = [vp, i32, i64]
+        L.fdas_plan_info.argtypes = [vp, C.POINTER(FdasInfo)]
+        L.fdas_build_templates.argtypes = [vp, vp]
+        L.fdas_get_templates.argtypes = [vp, vp]
+        L.fdas_spectrum.argtypes = [vp, vp, i32, vp, vp, vp, vp]
+        L.fdas_correlate.argtypes = [vp, vp, i32, vp, f32, vp, vp, u32, vp, vp]
+        L.fdas_harmsum.argtypes = [vp, vp, i32, vp, vp, vp, u32, vp]
+        L.fdas_candidates.argtypes = [vp, vp, f32, vp, vp, u32, vp]
+        L.fdas_search_host.argtypes = [vp, vp, i32, i32, vp, vp, vp, u32, vp]
+        L.fdas_threshold.argtypes = [i32, f64]
+        L.fdas_threshold.restype = f64
+        L.fdas_plan_destroy.argtypes = [vp]
+        L.fdas_strerror.argtypes = [C.c_int]
+        L.fdas_strerror.restype = C.c_char_p
+        for n in EXPORTS:
+            if n not in ("fdas_threshold", "fdas_strerror"):
+                getattr(L, n).restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _check(code, where):
+    if code != FDAS_OK:
+        raise FdasError(code, where)
+
+
+def _dptr(t):
+    return C.c_void_p(t.data_ptr()) if t is not None else None
+
+
+def _stream(stream=None):
+    s = stream if stream is not None else torch.cuda.current_stream()
+    return C.c_void_p(s.cuda_stream)
+
+
+# --------------------------------------------------------------------------- C-ABI mirrors
+def fdas_set_device(device: int):
+    _check(lib().fdas_set_device(int(device)), "fdas_set_device")
+
+
+def fdas_plan_create(n_samples, z_max, dz, template_width, segment_len):
+    h = C.c_void_p()
+    _check(lib().fdas_plan_create(C.byref(h), int(n_samples), float(z_max), float(dz),
+                                  int(template_width), int(segment_len)), "fdas_plan_create")
+    return h
+
+
+def fdas_plan_set_option(plan, key, value):
+    _check(lib().fdas_plan_set_option(plan, int(key), int(value)), "fdas_plan_set_option")
+
+
+def fdas_plan_info(plan) -> FdasInfo:
+    info = FdasInfo()
+    _check(lib().fdas_plan_info(plan, C.byref(info)), "fdas_plan_info")
+    return info
+
+
+def fdas_build_templates(plan, stream=None):
+    _check(lib().fdas_build_templates(plan, _stream(stream)), "fdas_build_templates")
+
+
+def fdas_get_templates(plan) -> np.ndarray:
+    info = fdas_plan_info(plan)
+    out = np.empty((info.n_templates, info.width, 2), dtype=np.float32)
+    _check(lib().fdas_get_templates(plan, out.ctypes.data_as(C.c_void_p)), "fdas_get_templates")
+    return out[..., 0] + 1j * out[..., 1]
+
+
+def fdas_spectrum(plan, d_series, n_batch, d_spectrum, d_meanpow, d_workspace, stream=None):
+    _check(lib().fdas_spectrum(plan, _dptr(d_series), int(n_batch), _dptr(d_spectrum), _dptr(d_meanpow),
+                               _dptr(d_workspace), _stream(stream)), "fdas_spectrum")
+
+
+def fdas_correlate(plan, d_spectrum, n_batch, d_plane, threshold, d_cands, d_counts, capacity,
+                   d_workspace=None, stream=None):
+    _check(lib().fdas_correlate(plan, _dptr(d_spectrum), int(n_batch), _dptr(d_plane), float(threshold),
+                                _dptr(d_cands), _dptr(d_counts), int(capacity), _dptr(d_workspace),
+                                _stream(stream)), "fdas_correlate")
+
+
+def fdas_harmsum(plan, d_plane, max_harm, thresholds, d_cands, d_count, capacity, stream=None):
+    thr = np.ascontiguousarray(thresholds, dtype=np.float32)
+    _check(lib().fdas_harmsum(plan, _dptr(d_plane), int(max_harm), thr.ctypes.data_as(C.c_void_p),
+                              _dptr(d_cands), _dptr(d_count), int(capacity), _stream(stream)), "fdas_harmsum")
+
+
+def fdas_candidates(plan, d_plane, threshold, d_cands, d_count, capacity, stream=None):
+    _check(lib().fdas_candidates(plan, _dptr(d_plane), float(threshold), _dptr(d_cands), _dptr(d_count),
+                                 int(capacity), _stream(stream)), "fdas_candidates")
+
+
+def fdas_search_host(plan, h_series: np.ndarray, max_harm, thresholds, capacity, h_cands=None, h_counts=None,
+                     stream=None):
+    """Host-buffer path: h_series float32[n_batch, N] (numpy or pinned torch CPU tensor)."""
+    if isinstance(h_series, torch.Tensor):
+        ptr, n_batch = h_series.data_ptr(), (h_series.shape[0] if h_series.dim() == 2 else 1)
+    else:
+        h_series = np.ascontiguousarray(h_series, dtype=np.float32)
+        ptr, n_batch = h_series.ctypes.data, (h_series.shape[0] if h_series.ndim == 2 else 1)
+    thr = np.ascontiguousarray(thresholds, dtype=np.float32)
+    if h_cands is None:
+        h_cands = np.zeros((n_batch, capacity), dtype=CAND_DTYPE)
+    if h_counts is None:
+        h_counts = np.zeros(n_batch, dtype=np.uint32)
+    _check(lib().fdas_search_host(plan, C.c_void_p(ptr), int(n_batch), int(max_harm),
+                                  thr.ctypes.data_as(C.c_void_p), h_cands.ctypes.data_as(C.c_void_p),
+                                  h_counts.ctypes.data_as(C.c_void_p), int(capacity), _stream(stream)),
+           "fdas_search_host")
+    return h_cands, h_counts
+
+
+def fdas_threshold(n_harm: int, pfa: float = 1e-6) -> float:
+    return lib().fdas_threshold(int(n_harm), float(pfa))
+
+
+def fdas_plan_destroy(plan):
+    _check(lib().fdas_plan_destroy(plan), "fdas_plan_destroy")
+
+
+def thresholds(max_harm: int, pfa: float = 1e-6) -> np.ndarray:
+    return np.array([fdas_threshold(1 << s, pfa) for s in range(int(max_harm).bit_length())], dtype=np.float64)
+
+
+# --------------------------------------------------------------------------- convenience
+class Plan:
+    """Owns an fdas_plan handle plus the torch device buffers the hot calls need."""
+
+    def __init__(self, n_samples, z_max, dz, template_width, segment_len, interbin=0, max_batch=1,
+                 quad_points=None, device=None):
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_1511_07343_b200 needs a CUDA device (no CPU fallback)")
+        self.device = torch.device("cuda", torch.cuda.current_device() if device is None else device)
+        fdas_set_device(self.device.index)
+        self.handle = fdas_plan_create(n_samples, z_max, dz, template_width, segment_len)
+        if interbin:
+            fdas_plan_set_option(self.handle, FDAS_OPT_INTERBIN, 1)
+        if max_batch != 1:
+            fdas_plan_set_option(self.handle, FDAS_OPT_MAX_BATCH, max_batch)
+        if quad_points:
+            fdas_plan_set_option(self.handle, FDAS_OPT_QUAD_POINTS, quad_points)
+        self.info = fdas_plan_info(self.handle)
+        self.max_batch = max_batch
+        fdas_build_templates(self.handle)
+        self.workspace = torch.empty(self.info.workspace_bytes, dtype=torch.uint8, device=self.device)
+
+    def close(self):
+        if self.handle is not None:
+            fdas_plan_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # buffers
+    def empty_spectrum(self, n_batch=1):
+        return torch.empty((n_batch, self.info.n_bins, 2), dtype=torch.float32, device=self.device)
+
+    def empty_plane(self, n_batch=1):
+        return torch.empty((n_batch, self.info.n_z, self.info.n_cols), dtype=torch.float32, device=self.device)
+
+    def empty_cands(self, capacity, n_batch=1):
+        return (torch.zeros((n_batch, capacity, 3), dtype=torch.int32, device=self.device),
+                torch.zeros(n_batch, dtype=torch.int32, device=self.device))
+
+    # calls
+    def spectrum(self, d_series, d_spectrum=None, d_meanpow=None, stream=None):
+        n_batch = d_series.shape[0] if d_series.dim() == 2 else 1
+        if d_spectrum is None:
+            d_spectrum = self.empty_spectrum(n_batch)
+        if d_meanpow is None:
+            d_meanpow = torch.empty(n_batch, dtype=torch.float32, device=self.device)
+        fdas_spectrum(self.handle, d_series, n_batch, d_spectrum, d_meanpow, self.workspace, stream)
+        return d_spectrum, d_meanpow
+
+    def correlate(self, d_spectrum, d_plane=None, threshold=0.0, cands=None, capacity=0, stream=None):
+        n_batch = d_spectrum.shape[0]
+        d_c, d_n = cands if cands is not None else (None, None)
+        fdas_correlate(self.handle, d_spectrum, n_batch, d_plane, threshold, d_c, d_n, capacity, None, stream)
+
+    def harmsum(self, d_plane, max_harm, thr, cands, capacity, stream=None):
+        fdas_harmsum(self.handle, d_plane, max_harm, thr, cands[0], cands[1], capacity, stream)
+
+    def candidates(self, d_plane, threshold, cands, capacity, stream=None):
+        fdas_candidates(self.handle, d_plane, threshold, cands[0], cands[1], capacity, stream)
+
+    def search_host(self, h_series, max_harm, thr, capacity, h_cands=None, h_counts=None, stream=None):
+        return fdas_search_host(self.handle, h_series, max_harm, thr, capacity, h_cands, h_counts, stream)
+
+
+def cands_to_numpy(d_cands, d_counts, b=0) -> np.ndarray:
+    """Device candidate buffer (int32[n_batch, cap, 3] view of 12-byte records) -> structured array."""
+    n = int(d_counts[b].item())
+    cap = d_cands.shape[1]
+    if n > cap:
+        raise OverflowError("candidate capacity %d < %d found" % (cap, n))
+    raw = d_cands[b, :n].contiguous().cpu().numpy()
+    return raw.view(CAND_DTYPE).reshape(-1)
