@@ -1,0 +1,187 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element
+on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
+  power:  |P_gpu - P_ref| <= 1e-4*max(P_ref) + 1e-5*P_ref
+  candidate (col, zi, nharm) sets identical except entries within 1e-4 relative of the threshold.
+"""
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from paper_1511_07343_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def fdas():
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_1511_07343_b200 import fdas as m
+    m.lib()
+    return m
+
+
+def assert_power_parity(P_gpu, P_ref, pmax=None):
+    P_ref = np.asarray(P_ref, dtype=np.float64)
+    pmax = float(P_ref.max()) if pmax is None else pmax
+    err = np.abs(np.asarray(P_gpu, dtype=np.float64) - P_ref)
+    tol = 1e-4 * pmax + 1e-5 * P_ref
+    bad = err > tol
+    assert not bad.any(), "max err %.3e (tol %.3e) at %s" % (err.max(), tol.flat[err.argmax()],
+                                                           np.unravel_index(err.argmax(), err.shape))
+    return float(err.max())
+
+
+def cand_set(c):
+    return {(int(r["nharm"]), int(r["zi"]), int(r["col"])) for r in c}
+
+
+def assert_cand_parity(c_gpu, c_ref, thr_of_nharm, val_ref=None):
+    """Sets equal except entries whose (reference) power is within 1e-4 relative of the threshold."""
+    g, r = cand_set(c_gpu), cand_set(c_ref)
+    assert len(c_gpu) == len(g), "duplicate candidates"
+    pw_ref = {(int(x["nharm"]), int(x["zi"]), int(x["col"])): float(x["power"]) for x in c_ref}
+    pw_gpu = {(int(x["nharm"]), int(x["zi"]), int(x["col"])): float(x["power"]) for x in c_gpu}
+    for key in g ^ r:
+        p = pw_ref.get(key, pw_gpu.get(key))
+        T = thr_of_nharm(key[0])
+        assert abs(p - T) <= 1e-4 * T, "candidate mismatch %s power %g thr %g" % (key, p, T)
+    pmax = max(pw_ref.values()) if pw_ref else 1.0
+    for key in g & r:
+        assert abs(pw_gpu[key] - pw_ref[key]) <= 1e-4 * pmax + 1e-5 * pw_ref[key]
+
+
+def make_plan(fdas, cfg, max_batch=1):
+    return fdas.Plan(cfg.n_samples, cfg.z_max, cfg.dz, cfg.width, cfg.seg_len, interbin=cfg.interbin,
+                     max_batch=max_batch)
+
+
+# ------------------------------------------------------------------ templates (row a0)
+@pytest.mark.parametrize("idx", [0, 1, 2])
+def test_templates_match_oracle(fdas, idx):
+    cfg = synth.config(idx)
+    plan = make_plan(fdas, cfg)
+    T_gpu = fdas.fdas_get_templates(plan.handle)
+    T_ref = oracle.templates(cfg.z_max, cfg.dz, cfg.width, cfg.interbin)
+    assert T_gpu.shape == T_ref.shape
+    assert np.max(np.abs(T_gpu - T_ref)) <= 1e-6
+
+
+# ------------------------------------------------------------------ spectrum (row a1)
+@pytest.mark.parametrize("log2n", [9, 10, 12, 13, 17, 20])
+def test_spectrum_matches_oracle(fdas, log2n):
+    N = 1 << log2n
+    L = 256
+    x = synth.make_series(N, 4242 + log2n, [synth.Signal(0.2, N / 8 + 0.3, 2.0, 0.5)])
+    x[: N // 2] += 3.0                                   # non-zero mean and a step: exercises the Parseval path
+    plan = fdas.Plan(N, 4.0, 2.0, 16, L)
+    d_x = torch.from_numpy(x).cuda()
+    d_S, d_mu = plan.spectrum(d_x.view(1, -1))
+    S_gpu = d_S.cpu().numpy()[0]
+    S_gpu = S_gpu[:, 0] + 1j * S_gpu[:, 1]
+    S_ref, mu = oracle.spectrum(x)
+    assert float(d_mu[0]) == pytest.approx(mu, rel=2e-6)
+    scale = np.sqrt(np.mean(np.abs(S_ref) ** 2))         # = 1
+    assert np.max(np.abs(S_gpu - S_ref)) <= 3e-6 * np.max(np.abs(S_ref)) + 2e-5 * scale
+
+
+def test_spectrum_batched(fdas):
+    N = 1 << 14
+    xs = np.stack([synth.make_series(N, 900 + b) * (1.0 + b) for b in range(3)])
+    plan = fdas.Plan(N, 4.0, 2.0, 16, 256, max_batch=3)
+    d_S, d_mu = plan.spectrum(torch.from_numpy(xs).cuda())
+    for b in range(3):
+        S_ref, mu = oracle.spectrum(xs[b])
+        S = d_S[b].cpu().numpy()
+        assert np.max(np.abs(S[:, 0] + 1j * S[:, 1] - S_ref)) < 2e-5
+        assert float(d_mu[b]) == pytest.approx(mu, rel=2e-6)
+
+
+# ------------------------------------------------------------------ correlate (rows a2-a6)
+def run_gpu_plane(fdas, plan, x, thr=None, cap=1 << 16):
+    d_x = torch.from_numpy(np.ascontiguousarray(x)).cuda().view(1, -1)
+    d_S, _ = plan.spectrum(d_x)
+    d_P = plan.empty_plane(1)
+    cands = plan.empty_cands(cap) if thr is not None else None
+    plan.correlate(d_S, d_P, threshold=thr or 0.0, cands=cands, capacity=cap if thr is not None else 0)
+    torch.cuda.synchronize()
+    c = fdas.cands_to_numpy(*cands) if thr is not None else None
+    return d_P[0], c
+
+
+def test_config0_plane_and_candidates(fdas):
+    cfg = synth.config(0)
+    x = cfg.series()
+    plan = make_plan(fdas, cfg)
+    d_P, c_gpu = run_gpu_plane(fdas, plan, x, thr=cfg.threshold)
+    S, mu = oracle.spectrum(x)
+    T = oracle.templates(cfg.z_max, cfg.dz, cfg.width)
+    P_ref = oracle.correlate_direct(S, T)                 # Eq. (1), the definition
+    assert_power_parity(d_P.cpu().numpy(), P_ref)
+    c_ref = oracle.candidates(P_ref, cfg.threshold)
+    assert len(c_ref) >= 3
+    assert_cand_parity(c_gpu, c_ref, lambda h: cfg.threshold)
+    # the injected signal peaks at its (r0, z): bin 10000, z = 8 (north_star)
+    zi, col = np.unravel_index(int(torch.argmax(d_P)), d_P.shape)
+    assert (-20 + 2 * zi, col + 1) == (8, 10000)
+
+
+@pytest.mark.parametrize("N,zmax,m,L,ib", [
+    (1 << 12, 6.0, 16, 256, 0), (1 << 12, 6.0, 16, 256, 1), (1 << 14, 10.0, 64, 512, 1),
+    (1 << 13, 8.0, 128, 256, 0), (1 << 15, 12.0, 32, 4096, 1), (1 << 14, 0.0, 2, 1024, 0),
+    (1 << 13, 8.0, 64, 2048, 1),
+])
+def test_small_configs_vs_direct_sum(fdas, N, zmax, m, L, ib):
+    cfg = synth.small_config(N, zmax, 2.0, m, L, interbin=ib, index=20 + ib)
+    x = cfg.series()
+    plan = make_plan(fdas, cfg)
+    d_P, c_gpu = run_gpu_plane(fdas, plan, x, thr=12.0)
+    S, _ = oracle.spectrum(x)
+    T = oracle.templates(zmax, 2.0, m, ib)
+    P_ref = oracle.correlate_direct(S, T, interbin=ib)
+    assert_power_parity(d_P.cpu().numpy(), P_ref)
+    assert_cand_parity(c_gpu, oracle.candidates(P_ref, 12.0), lambda h: 12.0)
+
+
+def test_fused_mode_and_overflow_count(fdas):
+    cfg = synth.config(0)
+    x = cfg.series()
+    plan = make_plan(fdas, cfg)
+    d_S, _ = plan.spectrum(torch.from_numpy(x).cuda().view(1, -1))
+    cands = plan.empty_cands(1 << 16)
+    plan.correlate(d_S, None, threshold=8.0, cands=cands, capacity=1 << 16)       # plane not stored
+    c_fused = fdas.cands_to_numpy(*cands)
+    d_P = plan.empty_plane(1)
+    plan.correlate(d_S, d_P)
+    c2 = plan.empty_cands(1 << 16)
+    plan.candidates(d_P[0], 8.0, c2, 1 << 16)                                      # fdas_candidates on the stored plane
+    c_plane = fdas.cands_to_numpy(*c2)
+    assert cand_set(c_fused) == cand_set(c_plane) and len(c_fused) > 100
+    P = d_P[0].cpu().numpy()
+    assert len(c_fused) == int((P > 8.0).sum())
+    for r in c_fused[:50]:
+        assert P[r["zi"], r["col"]] == r["power"]
+    # overflow: the count is the true number, only `capacity` records are written
+    small = plan.empty_cands(16)
+    plan.correlate(d_S, None, threshold=8.0, cands=small, capacity=16)
+    assert int(small[1][0]) == len(c_fused)
+
+
+# ------------------------------------------------------------------ harmonic sum (rows a7, a8)
+@pytest.mark.parametrize("max_harm", [1, 2, 4, 8, 16])
+def test_harmsum_random_plane(fdas, max_harm):
+    N = 1 << 13
+    plan = fdas.Plan(N, 8.0, 2.0, 16, 256)
+    n_z, n_cols = plan.info.n_z, plan.info.n_cols
+    rng = np.random.default_rng(77)
+    P = rng.exponential(1.0, size=(n_z, n_cols)).astype(np.float32)
+    P[4, 1000] = 40.0; P[6, 2001] = 35.0; P[1, 7] = 50.0
+    thr = oracle.thresholds(max_harm, 1e-3)
+    cands = plan.empty_cands(1 << 18)
+    plan.harmsum(torch.from_numpy(P).cuda(), max_harm, thr, cands, 1 << 18)
+    c_gpu = fdas.cands_to_numpy(*cands)
+    c_ref = oracle.harmsum(P.astype(np.float64), max_harm, thr, bin0=1)
+    assert len(c_ref) > 20
+    thr32 = thr.astype(np.float32)
+    assert_cand_parity(c_gpu, c_ref, lambda h: float(thr32[int(h).bit_length() - 1]))
