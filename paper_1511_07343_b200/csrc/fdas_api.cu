@@ -120,6 +120,7 @@ extern "C" int fdas_build_templates(fdas_plan* p, void* stream)
     if (!p->d_taps) {
         if (cudaMalloc(&p->d_taps, (size_t)p->n_t * p->m * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); return FDAS_E_NOMEM; }
         if (cudaMalloc(&p->d_W, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); return FDAS_E_NOMEM; }
+        if (cudaMalloc(&p->d_Wr, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); return FDAS_E_NOMEM; }
     }
     int rc = fdas_launch_templates(p, st);
     if (rc) return rc;

@@ -16,7 +16,8 @@ struct fdas_plan {
     size_t  ws_inter_bytes, ws_part_bytes, workspace_bytes;
     // template bank (device, owned)
     float2* d_taps;   // [n_t][m]  conj R_z(d_j), fp32
-    float2* d_W;      // [n_t][L]  FFT_L(index-reversed taps)/L, in the register layout of the segment kernel
+    float2* d_W;      // [n_t][L]  FFT_L(index-reversed taps)/L, natural order
+    float2* d_Wr;     // the same spectra in the register layout of k_correlate_2048 (L = 2048 only)
     // scratch arena of fdas_search_host (device, owned, lazily allocated)
     void*   arena;
     size_t  arena_bytes;
@@ -39,6 +40,7 @@ void fdas_set_cuda_error(cudaError_t e, const char* where);
 
 // kernel launchers (one per .cu file); all enqueue on `st` and return an FDAS code
 int fdas_launch_templates(fdas_plan* p, cudaStream_t st);
+int fdas_permute_templates(fdas_plan* p, cudaStream_t st);
 int fdas_launch_spectrum(fdas_plan* p, const float* d_series, int n_batch, float2* d_spec,
                          float* d_meanpow, void* d_ws, cudaStream_t st);
 int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float* d_plane, float thr,

@@ -4,6 +4,8 @@
 // outputs -> plane row and/or thresholded candidates.  Computes Eq. (1).
 #include "fdas_common.cuh"
 #include "fdas_smemfft.cuh"
+#include "fdas_regfft.cuh"
+#include <stdlib.h>
 
 // v0 (generic L, natural-order smem Stockham): one CTA per (segment, batch entry).
 // smem: X[L] | A[L] | B[L].
@@ -45,10 +47,182 @@ k_correlate_smem(const float2* __restrict__ spec, const float2* __restrict__ W, 
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------
+// v1, L = 2048: register-resident 16 x 16 x 8 FFTs, 128 threads (4 warps) per CTA, 16 points per
+// thread.  Index split (inverse, DIT):  k = 128 k1 + 8 k2 + k3,  t = t1 + 16 t2 + 256 t3:
+//   pass 1  thread (k2,k3): Y[k1] = X[k1] W[k1], 16-point DFT over k1 -> t1          (no twiddles)
+//   ex1     [k3][t1][k2] (pitch 17), intra-warp (a warp owns two k3 values)
+//   pass 2  thread (t1,k3): twiddle exp(2 pi i k2 t1/256), 16-point DFT over k2 -> t2
+//   ex2     [k3][t2][t1], block barrier
+//   pass 3  thread p = t1 + 16 t2 (two per thread): twiddle exp(2 pi i k3 p/2048), 8-point DFT
+//           over k3 -> t3;  |.|^2;  coalesced store of t = p + 256 t3 < step.
+// The forward transform of the window runs the same passes in reverse (once per segment) and
+// leaves X[128 k1 + 8 k2 + k3] in the registers pass 1 needs; the template spectra are stored
+// in that same register layout (Wr), so nothing is reordered in the template loop.
+// The segment spectrum X stays in registers across all templates ("data reuse").
+constexpr int V1_THREADS = 128;
+constexpr int V1_PITCH3 = 272;                 // float2 per k3 region: 16 rows of pitch 17
+constexpr int V1_BUF = 8 * V1_PITCH3;          // one exchange buffer (2176 float2)
+
+__device__ __noinline__ void push_cand_slow(fdas_cand* list, uint32_t* count, uint32_t cap,
+                                            int col, int zi, float power)
+{
+    push_cand(list, count, cap, col, zi, 1, power);
+}
+
+template <bool HAS_PLANE, bool HAS_CANDS>
+__global__ void __launch_bounds__(V1_THREADS, 3)
+k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
+                 fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
+                 int n_bins, int n_z, int nset, int m, int step, int t_chunk)
+{
+    constexpr int L = 2048;
+    __shared__ float2 sm[2 * V1_BUF];
+    const int tid = threadIdx.x;
+    const int lo = tid & 15, k3A = tid >> 4;
+    const int seg = blockIdx.x, bt = blockIdx.z;
+    const int n_t = n_z * nset;
+    const int t_begin = blockIdx.y * t_chunk, t_end = min(n_t, t_begin + t_chunk);
+    const int c0 = seg * step;
+    const float2* S = spec + (size_t)bt * n_bins;
+
+    float2 X[16];
+    {   // ---- forward FFT of the window (sign -), reverse pass order
+        float2* buf = sm;
+#pragma unroll
+        for (int g = 0; g < 2; g++) {
+            const int p = tid + 128 * g;
+            float2 u[8];
+#pragma unroll
+            for (int n3 = 0; n3 < 8; n3++) {
+                long long c = (long long)c0 - m / 2 + p + 256 * n3;
+                u[bitrev(n3, 3)] = (c >= 0 && c < n_bins) ? S[c] : make_float2(0.f, 0.f);
+            }
+            dit_const<8, -1>(u);
+#pragma unroll
+            for (int k3 = 0; k3 < 8; k3++) {
+                float2 val = k3 ? cmul(u[k3], twiddle(k3 * p, L, -1.0f)) : u[0];
+                buf[p + V1_PITCH3 * k3] = val;
+            }
+        }
+        __syncthreads();
+        float2 v[16];
+#pragma unroll
+        for (int n2 = 0; n2 < 16; n2++) v[bitrev(n2, 4)] = buf[lo + 16 * n2 + V1_PITCH3 * k3A];
+        dit_const<16, -1>(v);
+#pragma unroll
+        for (int k2 = 1; k2 < 16; k2++) v[k2] = cmul(v[k2], twiddle(k2 * lo, 256, -1.0f));
+        __syncwarp();
+#pragma unroll
+        for (int k2 = 0; k2 < 16; k2++) buf[k2 + 17 * lo + V1_PITCH3 * k3A] = v[k2];
+        __syncwarp();
+#pragma unroll
+        for (int n1 = 0; n1 < 16; n1++) v[bitrev(n1, 4)] = buf[lo + 17 * n1 + V1_PITCH3 * k3A];
+        dit_const<16, -1>(v);
+#pragma unroll
+        for (int k1 = 0; k1 < 16; k1++) X[k1] = v[k1];
+        __syncthreads();
+    }
+
+    // per-thread twiddles of the inverse passes (loop invariant)
+    float2 tw2[8], tw3[2][4];
+    make_tw<16>(tw2, lo, 256);
+    make_tw<8>(tw3[0], tid, L);
+    make_tw<8>(tw3[1], tid + 128, L);
+
+    const size_t n_cols = (size_t)n_bins * nset;
+    for (int t = t_begin; t < t_end; t++) {
+        float2* buf = sm + ((t - t_begin) & 1) * V1_BUF;
+        const float4* Wt = Wr + (size_t)t * (8 * V1_THREADS) + tid;
+        float2 v[16];
+        {
+            float4 w4[8];
+#pragma unroll
+            for (int j = 0; j < 8; j++) w4[j] = __ldg(Wt + j * V1_THREADS);
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                v[bitrev(2 * j, 4)] = cmul(X[2 * j], make_float2(w4[j].x, w4[j].y));
+                v[bitrev(2 * j + 1, 4)] = cmul(X[2 * j + 1], make_float2(w4[j].z, w4[j].w));
+            }
+        }
+        dit_const<16, +1>(v);                                                    // pass 1: k1 -> t1
+#pragma unroll
+        for (int t1 = 0; t1 < 16; t1++) buf[lo + 17 * t1 + V1_PITCH3 * k3A] = v[t1];
+        __syncwarp();
+#pragma unroll
+        for (int k2 = 0; k2 < 16; k2++) v[bitrev(k2, 4)] = buf[k2 + 17 * lo + V1_PITCH3 * k3A];
+        dit_tw<16>(v, tw2);                                                      // pass 2: k2 -> t2
+        __syncwarp();
+#pragma unroll
+        for (int t2 = 0; t2 < 16; t2++) buf[lo + 16 * t2 + V1_PITCH3 * k3A] = v[t2];
+        __syncthreads();
+        const int zi = t / nset, s = t - zi * nset;
+        float* prow = HAS_PLANE ? plane + ((size_t)bt * n_z + zi) * n_cols + s : nullptr;
+#pragma unroll
+        for (int g = 0; g < 2; g++) {
+            const int p = tid + 128 * g;
+            float2 u[8];
+#pragma unroll
+            for (int k3 = 0; k3 < 8; k3++) u[bitrev(k3, 3)] = buf[p + V1_PITCH3 * k3];
+            dit_tw<8>(u, tw3[g]);                                                // pass 3: k3 -> t3
+#pragma unroll
+            for (int t3 = 0; t3 < 8; t3++) {
+                const int o = p + 256 * t3;
+                const int c = c0 + o;
+                if (o < step && c < n_bins) {
+                    float pw = fmaf(u[t3].x, u[t3].x, u[t3].y * u[t3].y);
+                    if (HAS_PLANE) prow[c * nset] = pw;
+                    if (HAS_CANDS) {
+                        if (pw > thr) push_cand_slow(cands + (size_t)bt * cap, counts + bt, cap, c * nset + s, zi, pw);
+                    }
+                }
+            }
+        }
+    }
+}
+
+// Wr[(t*8 + j)*128 + tid] = (W[128(2j) + 8 k2 + k3], W[128(2j+1) + 8 k2 + k3]), tid = 16 k3 + k2.
+__global__ void k_permute_templates_2048(const float2* __restrict__ W, float4* __restrict__ Wr, int n_t)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_t * 8 * V1_THREADS) return;
+    int tid = i % V1_THREADS, j = (i / V1_THREADS) % 8, t = i / (8 * V1_THREADS);
+    int k2 = tid & 15, k3 = tid >> 4;
+    float2 a = W[(size_t)t * 2048 + 128 * (2 * j) + 8 * k2 + k3];
+    float2 b = W[(size_t)t * 2048 + 128 * (2 * j + 1) + 8 * k2 + k3];
+    Wr[i] = make_float4(a.x, a.y, b.x, b.y);
+}
+
+int fdas_permute_templates(fdas_plan* p, cudaStream_t st)
+{
+    if (p->L != 2048) return FDAS_OK;
+    int n = p->n_t * 8 * V1_THREADS;
+    k_permute_templates_2048<<<(n + 255) / 256, 256, 0, st>>>(p->d_W, reinterpret_cast<float4*>(p->d_Wr), p->n_t);
+    FDAS_LAUNCH_CHECK();
+    return FDAS_OK;
+}
+
 int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float* d_plane, float thr,
                           fdas_cand* d_cands, uint32_t* d_counts, uint32_t cap, cudaStream_t st)
 {
     if (d_cands) FDAS_CUDA(cudaMemsetAsync(d_counts, 0, sizeof(uint32_t) * n_batch, st));
+    static const bool force_v0 = getenv("FDAS_CORRELATE_V0") != nullptr;
+    if (p->L == 2048 && !force_v0) {
+        static const int env_chunks = getenv("FDAS_T_CHUNKS") ? atoi(getenv("FDAS_T_CHUNKS")) : 0;
+        int n_chunk = env_chunks > 0 ? env_chunks : 1;
+        int t_chunk = (p->n_t + n_chunk - 1) / n_chunk;
+        n_chunk = (p->n_t + t_chunk - 1) / t_chunk;
+        dim3 grid(p->n_seg, n_chunk, n_batch);
+#define FDAS_V1_ARGS d_spec, reinterpret_cast<const float4*>(p->d_Wr), d_plane, d_cands, d_counts, cap, thr, \
+                     (int)p->n_bins, p->n_z, p->nset, p->m, p->step, t_chunk
+        if (d_plane && d_cands) k_correlate_2048<true, true><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);
+        else if (d_plane) k_correlate_2048<true, false><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);
+        else k_correlate_2048<false, true><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);
+#undef FDAS_V1_ARGS
+        FDAS_LAUNCH_CHECK();
+        return FDAS_OK;
+    }
     size_t smem = 3 * (size_t)p->L * sizeof(float2);
     FDAS_CUDA(cudaFuncSetAttribute(k_correlate_smem, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_correlate_smem<<<dim3(p->n_seg, n_batch), 256, smem, st>>>(d_spec, p->d_W, d_plane, d_cands, d_counts, cap, thr,

@@ -107,6 +107,7 @@ extern "C" int fdas_plan_destroy(fdas_plan* p)
     if (!p) return FDAS_E_INVALID;
     if (p->d_taps) cudaFree(p->d_taps);
     if (p->d_W) cudaFree(p->d_W);
+    if (p->d_Wr) cudaFree(p->d_Wr);
     if (p->arena) cudaFree(p->arena);
     delete p;
     return FDAS_OK;

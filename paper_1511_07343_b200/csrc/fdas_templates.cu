@@ -71,5 +71,5 @@ int fdas_launch_templates(fdas_plan* p, cudaStream_t st)
     FDAS_CUDA(cudaFuncSetAttribute(k_template_spectrum, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k_template_spectrum<<<p->n_t, 256, smem, st>>>(p->d_taps, p->d_W, p->m, p->L, p->nset);
     FDAS_LAUNCH_CHECK();
-    return FDAS_OK;
+    return fdas_permute_templates(p, st);
 }
