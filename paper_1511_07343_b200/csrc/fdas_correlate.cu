@@ -71,13 +71,14 @@ __device__ __noinline__ void push_cand_slow(fdas_cand* list, uint32_t* count, ui
     push_cand(list, count, cap, col, zi, 1, power);
 }
 
-template <bool HAS_PLANE, bool HAS_CANDS>
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET>
 __global__ void __launch_bounds__(V1_THREADS, 3)
 k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
                  fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
-                 int n_bins, int n_z, int nset, int m, int step, int t_chunk)
+                 int n_bins, int n_z, int m, int step, int t_chunk)
 {
     constexpr int L = 2048;
+    constexpr int nset = NSET;
     __shared__ float2 sm[2 * V1_BUF];
     const int tid = threadIdx.x;
     const int lo = tid & 15, k3A = tid >> 4;
@@ -132,19 +133,27 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
     make_tw<8>(tw3[1], tid + 128, L);
 
     const size_t n_cols = (size_t)n_bins * nset;
+    // number of kept outputs t = p + 256 t3 < min(step, n_bins - c0) for this thread's two p values
+    const int omax = min(step, n_bins - c0);
+    int nv[2];
+#pragma unroll
+    for (int g = 0; g < 2; g++) nv[g] = max(0, min(8, (omax - (tid + 128 * g) + 255) >> 8));
+    float* pbase = HAS_PLANE ? plane + (size_t)bt * n_z * n_cols + (size_t)(c0 + tid) * nset : nullptr;
+
+    // template spectra are software-pipelined: W(t+1) is fetched while pass 3 of template t runs
+    float4 w4[8];
+    if (t_begin < t_end) {
+        const float4* Wt = Wr + (size_t)t_begin * (8 * V1_THREADS) + tid;
+#pragma unroll
+        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wt + j * V1_THREADS);
+    }
     for (int t = t_begin; t < t_end; t++) {
         float2* buf = sm + ((t - t_begin) & 1) * V1_BUF;
-        const float4* Wt = Wr + (size_t)t * (8 * V1_THREADS) + tid;
         float2 v[16];
-        {
-            float4 w4[8];
 #pragma unroll
-            for (int j = 0; j < 8; j++) w4[j] = __ldg(Wt + j * V1_THREADS);
-#pragma unroll
-            for (int j = 0; j < 8; j++) {
-                v[bitrev(2 * j, 4)] = cmul(X[2 * j], make_float2(w4[j].x, w4[j].y));
-                v[bitrev(2 * j + 1, 4)] = cmul(X[2 * j + 1], make_float2(w4[j].z, w4[j].w));
-            }
+        for (int j = 0; j < 8; j++) {
+            v[bitrev(2 * j, 4)] = cmul(X[2 * j], make_float2(w4[j].x, w4[j].y));
+            v[bitrev(2 * j + 1, 4)] = cmul(X[2 * j + 1], make_float2(w4[j].z, w4[j].w));
         }
         dit_const<16, +1>(v);                                                    // pass 1: k1 -> t1
 #pragma unroll
@@ -156,9 +165,14 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
         __syncwarp();
 #pragma unroll
         for (int t2 = 0; t2 < 16; t2++) buf[lo + 16 * t2 + V1_PITCH3 * k3A] = v[t2];
+        {
+            const float4* Wn = Wr + (size_t)min(t + 1, t_end - 1) * (8 * V1_THREADS) + tid;
+#pragma unroll
+            for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * V1_THREADS);
+        }
         __syncthreads();
-        const int zi = t / nset, s = t - zi * nset;
-        float* prow = HAS_PLANE ? plane + ((size_t)bt * n_z + zi) * n_cols + s : nullptr;
+        const int zi = NSET == 1 ? t : (t >> 1), s = NSET == 1 ? 0 : (t & 1);
+        float* prow = HAS_PLANE ? pbase + (size_t)zi * n_cols + s : nullptr;
 #pragma unroll
         for (int g = 0; g < 2; g++) {
             const int p = tid + 128 * g;
@@ -168,13 +182,12 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
             dit_tw<8>(u, tw3[g]);                                                // pass 3: k3 -> t3
 #pragma unroll
             for (int t3 = 0; t3 < 8; t3++) {
-                const int o = p + 256 * t3;
-                const int c = c0 + o;
-                if (o < step && c < n_bins) {
-                    float pw = fmaf(u[t3].x, u[t3].x, u[t3].y * u[t3].y);
-                    if (HAS_PLANE) prow[c * nset] = pw;
+                float pw = fmaf(u[t3].x, u[t3].x, u[t3].y * u[t3].y);
+                if (t3 < nv[g]) {
+                    if (HAS_PLANE) prow[(128 * g + 256 * t3) * NSET] = pw;
                     if (HAS_CANDS) {
-                        if (pw > thr) push_cand_slow(cands + (size_t)bt * cap, counts + bt, cap, c * nset + s, zi, pw);
+                        if (pw > thr)
+                            push_cand_slow(cands + (size_t)bt * cap, counts + bt, cap, (c0 + p + 256 * t3) * nset + s, zi, pw);
                     }
                 }
             }
@@ -210,15 +223,18 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
     static const bool force_v0 = getenv("FDAS_CORRELATE_V0") != nullptr;
     if (p->L == 2048 && !force_v0) {
         static const int env_chunks = getenv("FDAS_T_CHUNKS") ? atoi(getenv("FDAS_T_CHUNKS")) : 0;
-        int n_chunk = env_chunks > 0 ? env_chunks : 1;
+        int n_chunk = env_chunks > 0 ? env_chunks : (p->n_t + 28) / 29;      // ~29 templates per CTA: short tail
         int t_chunk = (p->n_t + n_chunk - 1) / n_chunk;
         n_chunk = (p->n_t + t_chunk - 1) / t_chunk;
         dim3 grid(p->n_seg, n_chunk, n_batch);
 #define FDAS_V1_ARGS d_spec, reinterpret_cast<const float4*>(p->d_Wr), d_plane, d_cands, d_counts, cap, thr, \
-                     (int)p->n_bins, p->n_z, p->nset, p->m, p->step, t_chunk
-        if (d_plane && d_cands) k_correlate_2048<true, true><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);
-        else if (d_plane) k_correlate_2048<true, false><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);
-        else k_correlate_2048<false, true><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);
+                     (int)p->n_bins, p->n_z, p->m, p->step, t_chunk
+#define FDAS_V1_LAUNCH(NS)                                                                                   \
+        if (d_plane && d_cands) k_correlate_2048<true, true, NS><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS); \
+        else if (d_plane) k_correlate_2048<true, false, NS><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);      \
+        else k_correlate_2048<false, true, NS><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS)
+        if (p->nset == 1) { FDAS_V1_LAUNCH(1); } else { FDAS_V1_LAUNCH(2); }
+#undef FDAS_V1_LAUNCH
 #undef FDAS_V1_ARGS
         FDAS_LAUNCH_CHECK();
         return FDAS_OK;
