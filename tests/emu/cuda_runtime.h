@@ -1,0 +1,90 @@
+// Host emulation shim for CUDA device code (dev tool, _work only).
+#pragma once
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#include <stdio.h>
+#include <functional>
+
+#define __global__
+#define __device__
+#define __host__
+#define __forceinline__ inline __attribute__((always_inline))
+#define __noinline__ __attribute__((noinline))
+#define __restrict__ __restrict
+#define __launch_bounds__(...)
+#define __shared__ thread_local
+
+struct float2 { float x, y; };
+struct alignas(16) float4 { float x, y, z, w; };
+struct double2 { double x, y; };
+struct uint3 { unsigned x, y, z; };
+struct dim3 {
+    unsigned x, y, z;
+    dim3(unsigned a = 1, unsigned b = 1, unsigned c = 1) : x(a), y(b), z(c) {}
+};
+static inline float2 make_float2(float x, float y) { return float2{x, y}; }
+static inline float4 make_float4(float x, float y, float z, float w) { return float4{x, y, z, w}; }
+
+extern thread_local uint3 threadIdx, blockIdx;
+extern thread_local dim3 blockDim, gridDim;
+
+typedef int cudaError_t;
+typedef void* cudaStream_t;
+enum { cudaSuccess = 0, cudaErrorMemoryAllocation = 2 };
+enum cudaMemcpyKind { cudaMemcpyHostToDevice = 1, cudaMemcpyDeviceToHost = 2, cudaMemcpyDeviceToDevice = 3 };
+enum cudaFuncAttribute { cudaFuncAttributeMaxDynamicSharedMemorySize = 8 };
+
+cudaError_t cudaMalloc(void** p, size_t n);
+template <class T> static inline cudaError_t cudaMalloc(T** p, size_t n) { return cudaMalloc((void**)p, n); }
+cudaError_t cudaFree(void* p);
+cudaError_t cudaMemcpy(void* d, const void* s, size_t n, cudaMemcpyKind k);
+cudaError_t cudaMemcpyAsync(void* d, const void* s, size_t n, cudaMemcpyKind k, cudaStream_t st);
+cudaError_t cudaMemsetAsync(void* d, int v, size_t n, cudaStream_t st);
+static inline cudaError_t cudaStreamSynchronize(cudaStream_t) { return cudaSuccess; }
+static inline cudaError_t cudaGetLastError() { return cudaSuccess; }
+static inline cudaError_t cudaSetDevice(int) { return cudaSuccess; }
+static inline const char* cudaGetErrorString(cudaError_t) { return "emu"; }
+template <class F> static inline cudaError_t cudaFuncSetAttribute(F, cudaFuncAttribute, int) { return cudaSuccess; }
+
+// ---- device runtime
+void emu_syncthreads();
+void emu_syncwarp();
+void* emu_dyn_smem();
+void emu_check_ptr(const void* p, size_t n, const char* what);
+void emu_launch(dim3 grid, dim3 block, size_t smem, const char* name, const std::function<void()>& body);
+#define __syncthreads() emu_syncthreads()
+#define __syncwarp() emu_syncwarp()
+
+template <class T> static inline T __ldg(const T* p)
+{
+    emu_check_ptr(p, sizeof(T), "__ldg");
+    return *p;
+}
+template <class T> static inline T __ldcs(const T* p)
+{
+    emu_check_ptr(p, sizeof(T), "__ldcs");
+    return *p;
+}
+static inline unsigned atomicAdd(unsigned* p, unsigned v) { return __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+
+static inline void sincospif(float x, float* s, float* c)
+{
+    double r = (double)x - 2.0 * floor((double)x * 0.5);
+    *s = (float)sin(M_PI * r);
+    *c = (float)cos(M_PI * r);
+}
+static inline void sincospi(double x, double* s, double* c)
+{
+    double r = x - 2.0 * floor(x * 0.5);
+    *s = sin(M_PI * r);
+    *c = cos(M_PI * r);
+}
+static inline int min(int a, int b) { return a < b ? a : b; }
+static inline int max(int a, int b) { return a > b ? a : b; }
+static inline long long min(long long a, long long b) { return a < b ? a : b; }
+static inline long long max(long long a, long long b) { return a > b ? a : b; }
+static inline unsigned min(unsigned a, unsigned b) { return a < b ? a : b; }
+static inline float min(float a, float b) { return fminf(a, b); }
+static inline float max(float a, float b) { return fmaxf(a, b); }

@@ -1,0 +1,227 @@
+// Host emulation runtime: guard-paged "device" memory + coroutine CTA scheduler (dev tool).
+#include "cuda_runtime.h"
+#include <signal.h>
+#include <sys/mman.h>
+#include <ucontext.h>
+#include <unistd.h>
+#include <atomic>
+#include <map>
+#include <mutex>
+#include <thread>
+#include <vector>
+
+thread_local uint3 threadIdx, blockIdx;
+thread_local dim3 blockDim, gridDim;
+
+// ------------------------------------------------------------------ memory
+struct Alloc { char* map; size_t map_len; char* user; size_t n; };
+static std::map<uintptr_t, Alloc> g_allocs;      // keyed by user pointer
+static std::mutex g_mu;
+static const size_t PG = 4096;
+static bool align_end() { const char* e = getenv("EMU_ALIGN"); return !(e && !strcmp(e, "start")); }
+
+static void* guarded_alloc(size_t n)
+{
+    size_t body = (n + PG - 1) / PG * PG;
+    if (body == 0) body = PG;
+    size_t len = body + 2 * PG;
+    char* m = (char*)mmap(nullptr, len, PROT_READ | PROT_WRITE, MAP_PRIVATE | MAP_ANONYMOUS, -1, 0);
+    if (m == MAP_FAILED) return nullptr;
+    mprotect(m, PG, PROT_NONE);
+    mprotect(m + PG + body, PG, PROT_NONE);
+    char* user = m + PG;
+    if (align_end()) user = m + PG + body - ((n + 15) / 16 * 16);
+    memset(m + PG, 0xA5, body);                  // poison: uninitialised reads give garbage, like the GPU
+    std::lock_guard<std::mutex> lk(g_mu);
+    g_allocs[(uintptr_t)user] = Alloc{m, len, user, n};
+    return user;
+}
+static void guarded_free(void* p)
+{
+    std::lock_guard<std::mutex> lk(g_mu);
+    auto it = g_allocs.find((uintptr_t)p);
+    if (it == g_allocs.end()) { fprintf(stderr, "EMU: free of unknown pointer %p\n", p); abort(); }
+    munmap(it->second.map, it->second.map_len);
+    g_allocs.erase(it);
+}
+cudaError_t cudaMalloc(void** p, size_t n) { *p = guarded_alloc(n); return *p ? cudaSuccess : cudaErrorMemoryAllocation; }
+cudaError_t cudaFree(void* p) { if (p) guarded_free(p); return cudaSuccess; }
+cudaError_t cudaMemcpy(void* d, const void* s, size_t n, cudaMemcpyKind) { memcpy(d, s, n); return cudaSuccess; }
+cudaError_t cudaMemcpyAsync(void* d, const void* s, size_t n, cudaMemcpyKind, cudaStream_t) { memcpy(d, s, n); return cudaSuccess; }
+cudaError_t cudaMemsetAsync(void* d, int v, size_t n, cudaStream_t) { memset(d, v, n); return cudaSuccess; }
+extern "C" void* emu_malloc(size_t n) { return guarded_alloc(n); }
+extern "C" void emu_free(void* p) { guarded_free(p); }
+
+static thread_local const char* t_kernel = "(host)";
+static void describe(const void* p)
+{
+    std::lock_guard<std::mutex> lk(g_mu);
+    uintptr_t a = (uintptr_t)p;
+    for (auto& kv : g_allocs) {
+        const Alloc& al = kv.second;
+        if (a >= (uintptr_t)al.map && a < (uintptr_t)al.map + al.map_len)
+            fprintf(stderr, "     address is %+lld bytes from the start of a %zu-byte allocation (end %+lld)\n",
+                    (long long)(a - (uintptr_t)al.user), al.n, (long long)(a - (uintptr_t)al.user - al.n));
+    }
+}
+void emu_check_ptr(const void* p, size_t n, const char* what)
+{
+    if ((uintptr_t)p % n) {
+        fprintf(stderr, "EMU: misaligned %s of %zu bytes at %p in %s block (%u,%u,%u) thread (%u,%u)\n", what, n, p,
+                t_kernel, blockIdx.x, blockIdx.y, blockIdx.z, threadIdx.x, threadIdx.y);
+        abort();
+    }
+}
+static void on_segv(int, siginfo_t* si, void*)
+{
+    fprintf(stderr, "EMU: illegal access at %p in %s block (%u,%u,%u) thread (%u,%u,%u)\n", si->si_addr, t_kernel,
+            blockIdx.x, blockIdx.y, blockIdx.z, threadIdx.x, threadIdx.y, threadIdx.z);
+    describe(si->si_addr);
+    _exit(99);
+}
+__attribute__((constructor)) static void install()
+{
+    static char altstack[1 << 16];
+    stack_t ss; ss.ss_sp = altstack; ss.ss_size = sizeof(altstack); ss.ss_flags = 0;
+    sigaltstack(&ss, nullptr);
+    struct sigaction sa; memset(&sa, 0, sizeof(sa));
+    sa.sa_sigaction = on_segv; sa.sa_flags = SA_SIGINFO | SA_ONSTACK;
+    sigaction(SIGSEGV, &sa, nullptr);
+    sigaction(SIGBUS, &sa, nullptr);
+}
+
+// ------------------------------------------------------------------ CTA scheduler
+enum { ST_RUN = 0, ST_BLOCK_BAR = 1, ST_WARP_BAR = 2, ST_DONE = 3 };
+struct Fiber { ucontext_t ctx; char* stack; int state; uint3 tid; };
+struct Worker {
+    std::vector<Fiber> fibers;
+    ucontext_t sched;
+    int cur;
+    const std::function<void()>* body;
+    void* dyn_smem;
+};
+static thread_local Worker* t_w = nullptr;
+static const size_t STACK = 256 << 10;
+
+static void tramp()
+{
+    Worker* w = t_w;
+    (*w->body)();
+    w = t_w;
+    w->fibers[w->cur].state = ST_DONE;
+    swapcontext(&w->fibers[w->cur].ctx, &w->sched);
+}
+static void yield_with(int st)
+{
+    Worker* w = t_w;
+    w->fibers[w->cur].state = st;
+    swapcontext(&w->fibers[w->cur].ctx, &w->sched);
+}
+void emu_syncthreads() { yield_with(ST_BLOCK_BAR); }
+void emu_syncwarp() { yield_with(ST_WARP_BAR); }
+void* emu_dyn_smem() { return t_w->dyn_smem; }
+
+static void run_block(Worker* w, dim3 block, bool rev)
+{
+    const int nt = block.x * block.y * block.z;
+    if ((int)w->fibers.size() < nt) {
+        size_t old = w->fibers.size();
+        w->fibers.resize(nt);
+        for (size_t i = old; i < (size_t)nt; i++) w->fibers[i].stack = (char*)guarded_alloc(STACK);
+    }
+    for (int i = 0; i < nt; i++) {
+        Fiber& f = w->fibers[i];
+        getcontext(&f.ctx);
+        f.ctx.uc_stack.ss_sp = f.stack;
+        f.ctx.uc_stack.ss_size = STACK;
+        f.ctx.uc_link = &w->sched;
+        makecontext(&f.ctx, tramp, 0);
+        f.state = ST_RUN;
+        f.tid = uint3{(unsigned)i % block.x, ((unsigned)i / block.x) % block.y, (unsigned)i / (block.x * block.y)};
+    }
+    int done = 0;
+    while (done < nt) {
+        bool progress = false;
+        for (int q = 0; q < nt; q++) {
+            int i = rev ? nt - 1 - q : q;
+            Fiber& f = w->fibers[i];
+            if (f.state != ST_RUN) continue;
+            w->cur = i;
+            threadIdx = f.tid;
+            swapcontext(&w->sched, &f.ctx);
+            progress = true;
+            if (f.state == ST_DONE) done++;
+        }
+        // release warp barriers
+        for (int w0 = 0; w0 < nt; w0 += 32) {
+            int at = 0, live = 0;
+            for (int i = w0; i < w0 + 32 && i < nt; i++) {
+                if (w->fibers[i].state != ST_DONE) live++;
+                if (w->fibers[i].state == ST_WARP_BAR) at++;
+            }
+            if (live && at == live) {
+                for (int i = w0; i < w0 + 32 && i < nt; i++)
+                    if (w->fibers[i].state == ST_WARP_BAR) w->fibers[i].state = ST_RUN;
+                progress = true;
+            }
+        }
+        int at = 0;
+        for (int i = 0; i < nt; i++) at += w->fibers[i].state == ST_BLOCK_BAR;
+        if (at && at == nt - done) {
+            for (int i = 0; i < nt; i++) if (w->fibers[i].state == ST_BLOCK_BAR) w->fibers[i].state = ST_RUN;
+            progress = true;
+        } else if (at && done && !progress) {
+            fprintf(stderr, "EMU: %s block (%u,%u,%u): __syncthreads reached by %d of %d threads after %d exited\n",
+                    t_kernel, blockIdx.x, blockIdx.y, blockIdx.z, at, nt, done);
+            abort();
+        }
+        if (!progress) {
+            fprintf(stderr, "EMU: deadlock in %s block (%u,%u,%u)\n", t_kernel, blockIdx.x, blockIdx.y, blockIdx.z);
+            abort();
+        }
+    }
+}
+
+static std::atomic<long> g_launches{0};
+extern "C" long emu_launch_count() { return g_launches.load(); }
+
+void emu_launch(dim3 grid, dim3 block, size_t smem, const char* name, const std::function<void()>& body)
+{
+    g_launches++;
+    if (getenv("EMU_TRACE"))
+        fprintf(stderr, "EMU launch %s grid (%u,%u,%u) block (%u,%u,%u) smem %zu\n", name, grid.x, grid.y, grid.z,
+                block.x, block.y, block.z, smem);
+    if ((size_t)block.x * block.y * block.z > 1024 || smem > 227 * 1024 || grid.y > 65535 || grid.z > 65535) {
+        fprintf(stderr, "EMU: invalid launch configuration for %s\n", name);
+        abort();
+    }
+    const long nblocks = (long)grid.x * grid.y * grid.z;
+    std::atomic<long> next{0};
+    const bool rev = getenv("EMU_ORDER") && !strcmp(getenv("EMU_ORDER"), "rev");
+    int nthr = getenv("EMU_THREADS") ? atoi(getenv("EMU_THREADS")) : (int)std::thread::hardware_concurrency();
+    if (nthr > nblocks) nthr = (int)nblocks;
+    if (nthr < 1) nthr = 1;
+    auto work = [&]() {
+        Worker* w = new Worker();
+        t_w = w;
+        t_kernel = name;
+        w->body = &body;
+        w->dyn_smem = smem ? guarded_alloc(smem) : nullptr;
+        gridDim = grid;
+        blockDim = block;
+        for (;;) {
+            long b = next.fetch_add(1);
+            if (b >= nblocks) break;
+            blockIdx = uint3{(unsigned)(b % grid.x), (unsigned)((b / grid.x) % grid.y), (unsigned)(b / ((long)grid.x * grid.y))};
+            run_block(w, block, rev);
+        }
+        if (w->dyn_smem) guarded_free(w->dyn_smem);
+        for (auto& f : w->fibers) guarded_free(f.stack);
+        delete w;
+        t_w = nullptr;
+        t_kernel = "(host)";
+    };
+    std::vector<std::thread> pool;
+    for (int i = 0; i < nthr; i++) pool.emplace_back(work);
+    for (auto& t : pool) t.join();
+}

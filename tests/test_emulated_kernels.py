@@ -1,0 +1,158 @@
+"""The CUDA kernels, run on the CPU: `tests/emu` compiles paper_1511_07343_b200/csrc/*.cu as host C++
+(one fibre per CUDA thread, real __syncthreads/__syncwarp semantics, guard pages around every "device"
+buffer and shared-memory array) and this file drives them through the product's own ctypes binding
+and compares with the fp64 oracle, exactly as tests/test_gpu_parity.py does on the B200.
+
+What this adds to the `-m gpu` tests: it runs where there is no GPU, and an out-of-bounds or
+misaligned access, a barrier reached by only part of a CTA, or a dependence on the order in which
+the threads of a CTA run (a missing barrier) fails here with the kernel, block and thread named,
+instead of raising an Xid on the GPU box.  It says nothing about speed.
+Test infrastructure only: nothing under paper_1511_07343_b200/ knows about it (tests/emu/README.md).
+"""
+import os
+import sys
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1511_07343_b200 import synth
+
+sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
+from emu import harness as E  # noqa: E402
+
+fdas = E.fdas
+
+
+@pytest.fixture(params=[("end", "fwd"), ("start", "rev")], ids=["guard-after", "guard-before-reversed"])
+def emu(request):
+    """Buffer placement against the trailing / leading guard page; thread order within a CTA forward / reversed."""
+    os.environ["EMU_ALIGN"], os.environ["EMU_ORDER"] = request.param
+    yield E
+    os.environ.pop("EMU_ALIGN"), os.environ.pop("EMU_ORDER")
+
+
+def power_ok(P_gpu, P_ref):
+    P_ref = np.asarray(P_ref, np.float64)
+    err = np.abs(np.asarray(P_gpu, np.float64) - P_ref)
+    assert not (err > 1e-4 * P_ref.max() + 1e-5 * P_ref).any(), err.max()
+
+
+def cset(c):
+    return {(int(r["nharm"]), int(r["zi"]), int(r["col"])) for r in c}
+
+
+def cand_ok(c_gpu, c_ref, thr_of):
+    g, r = cset(c_gpu), cset(c_ref)
+    assert len(c_gpu) == len(g), "duplicate candidates"
+    pw = {(int(x["nharm"]), int(x["zi"]), int(x["col"])): float(x["power"]) for x in list(c_gpu) + list(c_ref)}
+    for k in g ^ r:
+        assert abs(pw[k] - thr_of(k[0])) <= 1e-4 * thr_of(k[0]), k
+
+
+@pytest.mark.parametrize("log2n", [9, 10, 13, 16])
+def test_spectrum(emu, log2n):
+    N = 1 << log2n
+    x = synth.make_series(N, 4242 + log2n, [synth.Signal(0.2, N / 8 + 0.3, 2.0, 0.5)])
+    x[: N // 2] += 3.0
+    plan = emu.Plan(N, 4.0, 2.0, 16, 256, quad_points=64)
+    d_S, d_mu = plan.spectrum(x)
+    S = d_S.np()[0]
+    S_ref, mu = oracle.spectrum(x)
+    assert float(d_mu.np()[0]) == pytest.approx(mu, rel=2e-6)
+    assert np.max(np.abs(S[:, 0] + 1j * S[:, 1] - S_ref)) <= 3e-6 * np.max(np.abs(S_ref)) + 2e-5
+    plan.close()
+
+
+def test_spectrum_batched(emu):
+    N = 1 << 12
+    xs = np.stack([synth.make_series(N, 900 + b) * (1.0 + b) for b in range(3)])
+    plan = emu.Plan(N, 4.0, 2.0, 16, 256, max_batch=3, quad_points=64)
+    d_S, d_mu = plan.spectrum(xs)
+    for b in range(3):
+        S_ref, mu = oracle.spectrum(xs[b])
+        S = d_S.np()[b]
+        assert np.max(np.abs(S[:, 0] + 1j * S[:, 1] - S_ref)) < 2e-5
+        assert float(d_mu.np()[b]) == pytest.approx(mu, rel=2e-6)
+    plan.close()
+
+
+# (N, z_max, m, L, interbin): the generic shared-memory kernel (L != 2048) and every template
+# instance of the register-resident L = 2048 kernel, including a ragged last segment, m = L/2,
+# one template (z_max = 0) and more than one template chunk (n_t > 29).
+@pytest.mark.parametrize("N,zmax,m,L,ib", [
+    (1 << 12, 6.0, 16, 256, 1), (1 << 13, 8.0, 128, 256, 0), (1 << 14, 4.0, 32, 4096, 1), (1 << 12, 0.0, 2, 1024, 0),
+    (1 << 13, 8.0, 64, 2048, 1), (1 << 13, 8.0, 64, 2048, 0), (1 << 13, 60.0, 256, 2048, 0), (1 << 12, 2.0, 1024, 2048, 1),
+])
+def test_correlate_all_modes(emu, N, zmax, m, L, ib):
+    cfg = synth.small_config(N, zmax, 2.0, m, L, interbin=ib, index=20 + ib)
+    x = cfg.series()
+    plan = emu.Plan(N, zmax, 2.0, m, L, interbin=ib, quad_points=max(2048, 32 * m))
+    d_S, _ = plan.spectrum(x)
+    d_P, d_c, d_n = plan.correlate(d_S, True, 9.0, 1 << 14)           # plane + candidates
+    S, _ = oracle.spectrum(x)
+    T = oracle.templates(zmax, 2.0, m, ib)
+    assert np.max(np.abs(fdas.fdas_get_templates(plan.handle) - T)) <= 1e-6
+    P_ref = oracle.correlate_direct(S, T, interbin=ib)                 # Eq. (1), the definition
+    power_ok(d_P.np()[0], P_ref)
+    n = int(d_n.np()[0])
+    cand_ok(d_c.np()[0, :n], oracle.candidates(P_ref, 9.0), lambda h: 9.0)
+    _, d_c2, d_n2 = plan.correlate(d_S, False, 9.0, 1 << 14)          # fused: plane not stored
+    assert cset(d_c2.np()[0, :int(d_n2.np()[0])]) == cset(d_c.np()[0, :n])
+    d_P3, _, _ = plan.correlate(d_S, True)                            # plane only
+    assert np.array_equal(d_P3.np(), d_P.np())
+    _, _, d_n4 = plan.correlate(d_S, False, 9.0, 3)                   # overflow: true count, 3 records
+    assert int(d_n4.np()[0]) == n
+    c5, n5 = plan.candidates(d_P, 9.0, 1 << 14)                       # fdas_candidates on the stored plane
+    assert n5 == n and cset(c5) == cset(d_c.np()[0, :n])
+    plan.close()
+
+
+@pytest.mark.parametrize("N", [1 << 9, 1 << 12])
+@pytest.mark.parametrize("max_harm", [1, 2, 4, 8, 16])
+def test_harmsum(emu, N, max_harm):
+    plan = emu.Plan(N, 8.0, 2.0, 16, 256, quad_points=64)
+    n_z, n_cols = plan.info.n_z, plan.info.n_cols
+    P = np.random.default_rng(77).exponential(1.0, size=(n_z, n_cols)).astype(np.float32)
+    P[4, n_cols // 4] = 40.0; P[6, n_cols // 2 + 1] = 35.0; P[1, 7] = 50.0
+    thr = oracle.thresholds(max_harm, 1e-3)
+    c, n = plan.harmsum(E.to_dev(P), max_harm, thr, 1 << 16)
+    c_ref = oracle.harmsum(P.astype(np.float64), max_harm, thr, bin0=1)
+    assert len(c_ref) >= 3 and n == len(c)
+    thr32 = thr.astype(np.float32)
+    cand_ok(c, c_ref, lambda h: float(thr32[int(h).bit_length() - 1]))
+    plan.close()
+
+
+def test_fused_batch(emu):
+    small = synth.small_config(1 << 13, 8.0, 2.0, 64, 2048, n_dm=5, n_sig=1, index=33, amp=0.3)
+    xs = np.stack([small.series(d) for d in range(5)])
+    plan = emu.Plan(1 << 13, 8.0, 2.0, 64, 2048, max_batch=5, quad_points=2048)
+    d_S, _ = plan.spectrum(xs)
+    _, d_c, d_n = plan.correlate(d_S, False, 12.0, 1 << 10)
+    T = oracle.templates(8.0, 2.0, 64)
+    for d in range(5):
+        S, _ = oracle.spectrum(xs[d])
+        c_ref = oracle.candidates(oracle.correlate_direct(S, T), 12.0)
+        cand_ok(d_c.np()[d, :int(d_n.np()[d])], c_ref, lambda h: 12.0)
+    plan.close()
+
+
+def test_search_host(emu):
+    N = 1 << 13
+    cfg = synth.small_config(N, 8.0, 2.0, 64, 2048, n_sig=2, index=41, amp=0.3)
+    x = cfg.series()
+    plan = emu.Plan(N, 8.0, 2.0, 64, 2048, quad_points=2048)
+    thr = fdas.thresholds(8, 1e-3)
+    h_c, h_n = fdas.fdas_search_host(plan.handle, x.reshape(1, -1), 8, thr, 1 << 14)
+    d_S, _ = plan.spectrum(x)
+    d_P, _, _ = plan.correlate(d_S, True)
+    c, n = plan.harmsum(d_P, 8, thr, 1 << 14)
+    assert int(h_n[0]) == n and n > 0 and cset(h_c[0, :n]) == cset(c)
+    xs = np.stack([x, x[::-1].copy(), x])                             # batch larger than MAX_BATCH = 1
+    h_c, h_n = fdas.fdas_search_host(plan.handle, xs, 0, np.array([12.0]), 1 << 10)
+    c1, n1 = plan.candidates(d_P, 12.0, 1 << 10)
+    assert h_n[0] == h_n[2] == n1 and cset(h_c[0, :n1]) == cset(h_c[2, :n1]) == cset(c1)
+    h_c, h_n = fdas.fdas_search_host(plan.handle, xs, 4, fdas.thresholds(4, 1e-3), 1 << 14)
+    assert h_n[0] == h_n[2] and cset(h_c[0, :h_n[0]]) == cset(h_c[2, :h_n[2]])
+    plan.close()
