@@ -21,8 +21,11 @@ struct fdas_plan {
     // scratch arena of fdas_search_host (device, owned, lazily allocated)
     void*   arena;
     size_t  arena_bytes;
-    uint32_t arena_capacity;
-    int32_t  arena_batch;
+    uint32_t* pinned_counts;           // pinned host staging for the candidate counts
+    size_t  pinned_counts_n;
+    int32_t pipe_ready;                // copy streams + events of the host pipeline exist
+    cudaStream_t st_h2d, st_d2h;
+    cudaEvent_t ev_in[2], ev_free[2], ev_done[2];
 };
 
 void fdas_set_cuda_error(cudaError_t e, const char* where);

@@ -195,6 +195,167 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// v2, L = 2048: same 16 x 16 x 8 register-resident scheme and index split as v1, with fewer
+// instructions per (segment, template) in the loop (cuobjdump: see DESIGN.md section 6.1):
+//   * the template multiply is folded into the first butterfly stage (mul_first_stage16);
+//   * exchange 1 rows have pitch 18 float2 (16-byte aligned), so pass 2 reads its 16 inputs with
+//     8 LDS.128 (quarter-warp bank pattern 4 lo + 4 j: conflict-free);
+//   * pass 3 owns the ADJACENT outputs p = 2 tid, 2 tid + 1: 8 LDS.128 from exchange 2, and for
+//     integer-bin planes 8-byte stores of two neighbouring columns;
+//   * FAST (launched when step is a multiple of 256): a full segment keeps exactly t3 < step/256
+//     for every thread, so its stores are unpredicated and the butterflies feeding the discarded
+//     t3 = 7 outputs are dead code; the ragged last segment takes the predicated path.
+constexpr int V2_PITCH3 = 288;                 // float2 per k3 region: 16 rows of pitch 18
+constexpr int V2_BUF = 8 * V2_PITCH3;
+
+// Pass 3 of one template for this thread's outputs p = 2 tid (u0) and 2 tid + 1 (u1), t = p + 256 t3:
+// 8 LDS.128 from exchange 2, two 8-point DITs over k3, |.|^2, store / threshold.
+// FULL (CTA-uniform): every thread keeps exactly t3 < NKEEP, so nothing is predicated and the work
+// feeding t3 >= NKEEP is dead code; otherwise t3 < nv (ragged last segment, or step not a multiple of 256).
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool FULL>
+__device__ __forceinline__ void v2_pass3(const float2* buf, const float2* tw_a, const float2* tw_b, int tid,
+                                         float* prow, int nv, fdas_cand* cands, uint32_t* counts, uint32_t cap,
+                                         float thr, int col0, int zi)
+{
+    float2 u0[8], u1[8];
+#pragma unroll
+    for (int k3 = 0; k3 < 8; k3++) {
+        const float4 q = *reinterpret_cast<const float4*>(buf + 2 * tid + V2_PITCH3 * k3);
+        u0[bitrev(k3, 3)] = make_float2(q.x, q.y);
+        u1[bitrev(k3, 3)] = make_float2(q.z, q.w);
+    }
+    dit_tw<8>(u0, tw_a);
+    dit_tw<8>(u1, tw_b);
+#pragma unroll
+    for (int t3 = 0; t3 < 8; t3++) {
+        if (FULL ? (t3 >= NKEEP) : (t3 >= nv)) continue;
+        const float pa = fmaf(u0[t3].x, u0[t3].x, u0[t3].y * u0[t3].y);
+        const float pb = fmaf(u1[t3].x, u1[t3].x, u1[t3].y * u1[t3].y);
+        if (HAS_PLANE) {
+            if (NSET == 1) *reinterpret_cast<float2*>(prow + 256 * t3) = make_float2(pa, pb);
+            else { prow[(256 * t3) * NSET] = pa; prow[(256 * t3 + 1) * NSET] = pb; }
+        }
+        if (HAS_CANDS) {
+            if (pa > thr) push_cand_slow(cands, counts, cap, col0 + 256 * t3 * NSET, zi, pa);
+            if (pb > thr) push_cand_slow(cands, counts, cap, col0 + (256 * t3 + 1) * NSET, zi, pb);
+        }
+    }
+}
+
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP>
+__global__ void __launch_bounds__(V1_THREADS, 3)
+k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
+                    fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
+                    int n_bins, int n_z, int m, int step, int t_chunk)
+{
+    constexpr int L = 2048;
+    constexpr int nset = NSET;
+    __shared__ __align__(16) float2 sm[2 * V2_BUF];
+    const int tid = threadIdx.x;
+    const int lo = tid & 15, k3A = tid >> 4;
+    const int seg = blockIdx.x, bt = blockIdx.z;
+    const int n_t = n_z * nset;
+    const int t_begin = blockIdx.y * t_chunk, t_end = min(n_t, t_begin + t_chunk);
+    const int c0 = seg * step;
+    const float2* S = spec + (size_t)bt * n_bins;
+
+    float2 X[16];
+    {   // ---- forward FFT of the window (sign -), reverse pass order (as v1)
+        float2* buf = sm;
+#pragma unroll
+        for (int g = 0; g < 2; g++) {
+            const int p = tid + 128 * g;
+            float2 u[8];
+#pragma unroll
+            for (int n3 = 0; n3 < 8; n3++) {
+                long long c = (long long)c0 - m / 2 + p + 256 * n3;
+                u[bitrev(n3, 3)] = (c >= 0 && c < n_bins) ? S[c] : make_float2(0.f, 0.f);
+            }
+            dit_const<8, -1>(u);
+#pragma unroll
+            for (int k3 = 0; k3 < 8; k3++) {
+                float2 val = k3 ? cmul(u[k3], twiddle(k3 * p, L, -1.0f)) : u[0];
+                buf[p + V2_PITCH3 * k3] = val;
+            }
+        }
+        __syncthreads();
+        float2 v[16];
+#pragma unroll
+        for (int n2 = 0; n2 < 16; n2++) v[bitrev(n2, 4)] = buf[lo + 16 * n2 + V2_PITCH3 * k3A];
+        dit_const<16, -1>(v);
+#pragma unroll
+        for (int k2 = 1; k2 < 16; k2++) v[k2] = cmul(v[k2], twiddle(k2 * lo, 256, -1.0f));
+        __syncwarp();
+#pragma unroll
+        for (int k2 = 0; k2 < 16; k2++) buf[k2 + 18 * lo + V2_PITCH3 * k3A] = v[k2];
+        __syncwarp();
+#pragma unroll
+        for (int n1 = 0; n1 < 16; n1++) v[bitrev(n1, 4)] = buf[lo + 18 * n1 + V2_PITCH3 * k3A];
+        dit_const<16, -1>(v);
+#pragma unroll
+        for (int k1 = 0; k1 < 16; k1++) X[k1] = v[k1];
+        __syncthreads();
+    }
+
+    float2 tw2[8], tw3[2][4];
+    make_tw<16>(tw2, lo, 256);
+    make_tw<8>(tw3[0], 2 * tid, L);
+    make_tw<8>(tw3[1], 2 * tid + 1, L);
+
+    const size_t n_cols = (size_t)n_bins * nset;
+    const int omax = min(step, n_bins - c0);                       // even: step, n_bins and c0 are even
+    const bool full = (NKEEP < 8) && omax == step;                 // CTA-uniform
+    const int nv = max(0, min(8, (omax - 2 * tid + 255) >> 8));    // kept t3 of BOTH p = 2 tid and 2 tid + 1
+    float* pbase = HAS_PLANE ? plane + (size_t)bt * n_z * n_cols + (size_t)(c0 + 2 * tid) * nset : nullptr;
+    fdas_cand* clist = HAS_CANDS ? cands + (size_t)bt * cap : nullptr;
+    uint32_t* ccount = HAS_CANDS ? counts + bt : nullptr;
+
+    float4 w4[8];
+    const float4* Wn = Wr + (size_t)t_begin * (8 * V1_THREADS) + tid;      // template whose spectrum is fetched next
+    if (t_begin < t_end) {
+#pragma unroll
+        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * V1_THREADS);
+    }
+    float* prow1 = HAS_PLANE ? pbase + (size_t)t_begin * n_cols : nullptr;  // NSET == 1: row of template t
+    for (int t = t_begin; t < t_end; t++) {
+        float2* buf = sm + ((t - t_begin) & 1) * V2_BUF;
+        float2 v[16];
+        mul_first_stage16(v, X, w4);                                             // X W and stage 1
+        dit_const_stage<16, +1, 2>(v);                                           // pass 1: k1 -> t1
+        dit_const_stage<16, +1, 3>(v);
+        dit_const_stage<16, +1, 4>(v);
+#pragma unroll
+        for (int t1 = 0; t1 < 16; t1++) buf[lo + 18 * t1 + V2_PITCH3 * k3A] = v[t1];
+        __syncwarp();
+        {
+            const float4* row = reinterpret_cast<const float4*>(buf + 18 * lo + V2_PITCH3 * k3A);
+#pragma unroll
+            for (int j = 0; j < 8; j++) {
+                const float4 q = row[j];
+                v[bitrev(2 * j, 4)] = make_float2(q.x, q.y);
+                v[bitrev(2 * j + 1, 4)] = make_float2(q.z, q.w);
+            }
+        }
+        dit_tw<16>(v, tw2);                                                      // pass 2: k2 -> t2
+        __syncwarp();
+#pragma unroll
+        for (int t2 = 0; t2 < 16; t2++) buf[lo + 16 * t2 + V2_PITCH3 * k3A] = v[t2];
+        if (t + 1 < t_end) Wn += 8 * V1_THREADS;                                 // (the last iteration re-reads its own)
+#pragma unroll
+        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * V1_THREADS);
+        __syncthreads();
+        const int zi = NSET == 1 ? t : (t >> 1), s = NSET == 1 ? 0 : (t & 1);
+        float* prow = !HAS_PLANE ? nullptr : NSET == 1 ? prow1 : pbase + (size_t)zi * n_cols + s;
+        if (HAS_PLANE && NSET == 1) prow1 += n_cols;
+        const int col0 = (c0 + 2 * tid) * nset + s;
+        if (full)                                                                // pass 3: k3 -> t3
+            v2_pass3<HAS_PLANE, HAS_CANDS, NSET, NKEEP, true>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
+        else
+            v2_pass3<HAS_PLANE, HAS_CANDS, NSET, 8, false>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
+    }
+}
+
 // Wr[(t*8 + j)*128 + tid] = (W[128(2j) + 8 k2 + k3], W[128(2j+1) + 8 k2 + k3]), tid = 16 k3 + k2.
 __global__ void k_permute_templates_2048(const float2* __restrict__ W, float4* __restrict__ Wr, int n_t)
 {
@@ -229,11 +390,18 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
         dim3 grid(p->n_seg, n_chunk, n_batch);
 #define FDAS_V1_ARGS d_spec, reinterpret_cast<const float4*>(p->d_Wr), d_plane, d_cands, d_counts, cap, thr, \
                      (int)p->n_bins, p->n_z, p->m, p->step, t_chunk
-#define FDAS_V1_LAUNCH(NS)                                                                                   \
-        if (d_plane && d_cands) k_correlate_2048<true, true, NS><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS); \
-        else if (d_plane) k_correlate_2048<true, false, NS><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);      \
-        else k_correlate_2048<false, true, NS><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS)
-        if (p->nset == 1) { FDAS_V1_LAUNCH(1); } else { FDAS_V1_LAUNCH(2); }
+#define FDAS_V1_LAUNCH(K, ...)                                                                      \
+        if (d_plane && d_cands) K<true, true, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS); \
+        else if (d_plane) K<true, false, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);      \
+        else K<false, true, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS)
+        static const bool use_v1 = getenv("FDAS_CORRELATE_V1") != nullptr;
+        if (use_v1) {
+            if (p->nset == 1) { FDAS_V1_LAUNCH(k_correlate_2048, 1); } else { FDAS_V1_LAUNCH(k_correlate_2048, 2); }
+        } else if (p->step == 7 * 256) {                          // m = 256: full segments keep t3 < 7 exactly
+            if (p->nset == 1) { FDAS_V1_LAUNCH(k_correlate_2048_v2, 1, 7); } else { FDAS_V1_LAUNCH(k_correlate_2048_v2, 2, 7); }
+        } else {
+            if (p->nset == 1) { FDAS_V1_LAUNCH(k_correlate_2048_v2, 1, 8); } else { FDAS_V1_LAUNCH(k_correlate_2048_v2, 2, 8); }
+        }
 #undef FDAS_V1_LAUNCH
 #undef FDAS_V1_ARGS
         FDAS_LAUNCH_CHECK();

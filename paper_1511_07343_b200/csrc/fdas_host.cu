@@ -7,16 +7,19 @@
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// Scratch of fdas_search_host (all owned by the plan, built lazily): a device arena with TWO
+// series buffers (so the copy of chunk c+1 overlaps the kernels of chunk c: PAPER.md:49 step 1,
+// "asynchronous copy of the time series"), one spectrum, the FFT workspace, one plane
+// (harmonic-sum mode), candidate lists for the whole batch; two copy streams and a few events.
 struct Arena {
-    float* series; float* spec; void* ws; float* plane; fdas_cand* cands; uint32_t* counts;
+    float* series[2]; float* spec; void* ws; float* plane; fdas_cand* cands; uint32_t* counts;
 };
 
-// Carve the plan-owned arena: one chunk of `cb` series/spectra, one plane (harmonic-sum mode),
-// candidate lists for the whole batch.
 static int arena_prepare(fdas_plan* p, int n_batch, int cb, bool need_plane, uint32_t cap, Arena* a)
 {
+    const size_t series_b = align_up((size_t)cb * p->n_samples * sizeof(float), 256);
     size_t o_series = 0;
-    size_t o_spec = o_series + align_up((size_t)cb * p->n_samples * sizeof(float), 256);
+    size_t o_spec = o_series + 2 * series_b;
     size_t o_ws = o_spec + align_up((size_t)cb * p->n_bins * sizeof(float2), 256);
     size_t o_plane = o_ws + align_up(p->workspace_bytes, 256);
     size_t o_cands = o_plane + (need_plane ? align_up((size_t)p->n_z * p->n_cols * sizeof(float), 256) : 0);
@@ -28,13 +31,44 @@ static int arena_prepare(fdas_plan* p, int n_batch, int cb, bool need_plane, uin
         if (cudaMalloc(&p->arena, total) != cudaSuccess) { cudaGetLastError(); return FDAS_E_NOMEM; }
         p->arena_bytes = total;
     }
+    if ((size_t)n_batch > p->pinned_counts_n) {
+        if (p->pinned_counts) cudaFreeHost(p->pinned_counts);
+        p->pinned_counts = nullptr; p->pinned_counts_n = 0;
+        if (cudaMallocHost(&p->pinned_counts, (size_t)n_batch * sizeof(uint32_t)) != cudaSuccess) { cudaGetLastError(); return FDAS_E_NOMEM; }
+        p->pinned_counts_n = (size_t)n_batch;
+    }
+    if (!p->pipe_ready) {
+        FDAS_CUDA(cudaStreamCreateWithFlags(&p->st_h2d, cudaStreamNonBlocking));
+        FDAS_CUDA(cudaStreamCreateWithFlags(&p->st_d2h, cudaStreamNonBlocking));
+        for (int i = 0; i < 2; i++) {
+            FDAS_CUDA(cudaEventCreateWithFlags(&p->ev_in[i], cudaEventDisableTiming));
+            FDAS_CUDA(cudaEventCreateWithFlags(&p->ev_free[i], cudaEventDisableTiming));
+            FDAS_CUDA(cudaEventCreateWithFlags(&p->ev_done[i], cudaEventDisableTiming));
+        }
+        p->pipe_ready = 1;
+    }
     char* b = reinterpret_cast<char*>(p->arena);
-    a->series = reinterpret_cast<float*>(b + o_series);
+    a->series[0] = reinterpret_cast<float*>(b + o_series);
+    a->series[1] = reinterpret_cast<float*>(b + o_series + series_b);
     a->spec = reinterpret_cast<float*>(b + o_spec);
     a->ws = b + o_ws;
     a->plane = need_plane ? reinterpret_cast<float*>(b + o_plane) : nullptr;
     a->cands = reinterpret_cast<fdas_cand*>(b + o_cands);
     a->counts = reinterpret_cast<uint32_t*>(b + o_counts);
+    return FDAS_OK;
+}
+
+// Copy the candidate lists of series [b0, b0 + nb) back: their counts are already in pinned host memory.
+static int fetch_cands(fdas_plan* p, const Arena& a, int b0, int nb, uint32_t capacity, fdas_cand* h_cands,
+                       uint32_t* h_counts)
+{
+    for (int b = b0; b < b0 + nb; b++) {
+        h_counts[b] = p->pinned_counts[b];
+        uint32_t n = h_counts[b] < capacity ? h_counts[b] : capacity;
+        if (n)
+            FDAS_CUDA(cudaMemcpyAsync(h_cands + (size_t)b * capacity, a.cands + (size_t)b * capacity,
+                                      (size_t)n * sizeof(fdas_cand), cudaMemcpyDeviceToHost, p->st_d2h));
+    }
     return FDAS_OK;
 }
 
@@ -48,16 +82,31 @@ extern "C" int fdas_search_host(fdas_plan* p, const float* h_series, int32_t n_b
     if (!p->built) return FDAS_E_STATE;
     cudaStream_t st = (cudaStream_t)stream;
     const bool fused = (max_harm == 0);
-    const int cb = fused ? (n_batch < p->max_batch ? n_batch : p->max_batch) : 1;
+    const int cb = fused ? (n_batch < p->max_batch ? n_batch : p->max_batch) : 1;      // series per chunk
+    const int n_chunk = (n_batch + cb - 1) / cb;
     Arena a;
     int rc = arena_prepare(p, n_batch, cb, !fused, capacity, &a);
     if (rc) return rc;
-    for (int b0 = 0; b0 < n_batch; b0 += cb) {
-        int nb = n_batch - b0 < cb ? n_batch - b0 : cb;
-        FDAS_CUDA(cudaMemcpyAsync(a.series, h_series + (size_t)b0 * p->n_samples,
-                                  (size_t)nb * p->n_samples * sizeof(float), cudaMemcpyHostToDevice, st));
-        rc = fdas_launch_spectrum(p, a.series, nb, reinterpret_cast<float2*>(a.spec), nullptr, a.ws, st);
+    auto chunk_nb = [&](int c) { int b0 = c * cb; return n_batch - b0 < cb ? n_batch - b0 : cb; };
+    auto enqueue_h2d = [&](int c) -> int {       // on the copy stream, after the buffer's previous reader
+        if (c >= 2) FDAS_CUDA(cudaStreamWaitEvent(p->st_h2d, p->ev_free[c & 1], 0));
+        FDAS_CUDA(cudaMemcpyAsync(a.series[c & 1], h_series + (size_t)c * cb * p->n_samples,
+                                  (size_t)chunk_nb(c) * p->n_samples * sizeof(float), cudaMemcpyHostToDevice, p->st_h2d));
+        FDAS_CUDA(cudaEventRecord(p->ev_in[c & 1], p->st_h2d));
+        return FDAS_OK;
+    };
+    // the arena may still be in use by work the caller enqueued on `st` before this call
+    FDAS_CUDA(cudaEventRecord(p->ev_done[0], st));
+    FDAS_CUDA(cudaStreamWaitEvent(p->st_h2d, p->ev_done[0], 0));
+    rc = enqueue_h2d(0);
+    if (rc) return rc;
+    for (int c = 0; c < n_chunk; c++) {
+        const int b0 = c * cb, nb = chunk_nb(c);
+        if (c + 1 < n_chunk) { rc = enqueue_h2d(c + 1); if (rc) return rc; }
+        FDAS_CUDA(cudaStreamWaitEvent(st, p->ev_in[c & 1], 0));
+        rc = fdas_launch_spectrum(p, a.series[c & 1], nb, reinterpret_cast<float2*>(a.spec), nullptr, a.ws, st);
         if (rc) return rc;
+        FDAS_CUDA(cudaEventRecord(p->ev_free[c & 1], st));
         if (fused) {
             rc = fdas_launch_correlate(p, reinterpret_cast<const float2*>(a.spec), nb, nullptr, h_thresholds[0],
                                        a.cands + (size_t)b0 * capacity, a.counts + b0, capacity, st);
@@ -69,15 +118,19 @@ extern "C" int fdas_search_host(fdas_plan* p, const float* h_series, int32_t n_b
                                      a.counts + b0, capacity, st);
             if (rc) return rc;
         }
+        FDAS_CUDA(cudaMemcpyAsync(p->pinned_counts + b0, a.counts + b0, (size_t)nb * sizeof(uint32_t),
+                                  cudaMemcpyDeviceToHost, st));
+        FDAS_CUDA(cudaEventRecord(p->ev_done[c & 1], st));
+        if (c >= 1) {                             // one chunk behind: its lists come back while chunk c computes
+            FDAS_CUDA(cudaEventSynchronize(p->ev_done[(c - 1) & 1]));
+            rc = fetch_cands(p, a, (c - 1) * cb, chunk_nb(c - 1), capacity, h_cands, h_counts);
+            if (rc) return rc;
+        }
     }
-    FDAS_CUDA(cudaMemcpyAsync(h_counts, a.counts, (size_t)n_batch * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
-    FDAS_CUDA(cudaStreamSynchronize(st));
-    for (int b = 0; b < n_batch; b++) {
-        uint32_t n = h_counts[b] < capacity ? h_counts[b] : capacity;
-        if (n)
-            FDAS_CUDA(cudaMemcpyAsync(h_cands + (size_t)b * capacity, a.cands + (size_t)b * capacity,
-                                      (size_t)n * sizeof(fdas_cand), cudaMemcpyDeviceToHost, st));
-    }
+    FDAS_CUDA(cudaEventSynchronize(p->ev_done[(n_chunk - 1) & 1]));
+    rc = fetch_cands(p, a, (n_chunk - 1) * cb, chunk_nb(n_chunk - 1), capacity, h_cands, h_counts);
+    if (rc) return rc;
+    FDAS_CUDA(cudaStreamSynchronize(p->st_d2h));
     FDAS_CUDA(cudaStreamSynchronize(st));
     return FDAS_OK;
 }
@@ -109,6 +162,12 @@ extern "C" int fdas_plan_destroy(fdas_plan* p)
     if (p->d_W) cudaFree(p->d_W);
     if (p->d_Wr) cudaFree(p->d_Wr);
     if (p->arena) cudaFree(p->arena);
+    if (p->pinned_counts) cudaFreeHost(p->pinned_counts);
+    if (p->pipe_ready) {
+        cudaStreamDestroy(p->st_h2d);
+        cudaStreamDestroy(p->st_d2h);
+        for (int i = 0; i < 2; i++) { cudaEventDestroy(p->ev_in[i]); cudaEventDestroy(p->ev_free[i]); cudaEventDestroy(p->ev_done[i]); }
+    }
     delete p;
     return FDAS_OK;
 }

@@ -82,7 +82,7 @@ def test_spectrum_batched(emu):
 # one template (z_max = 0) and more than one template chunk (n_t > 29).
 @pytest.mark.parametrize("N,zmax,m,L,ib", [
     (1 << 12, 6.0, 16, 256, 1), (1 << 13, 8.0, 128, 256, 0), (1 << 14, 4.0, 32, 4096, 1), (1 << 12, 0.0, 2, 1024, 0),
-    (1 << 13, 8.0, 64, 2048, 1), (1 << 13, 8.0, 64, 2048, 0), (1 << 13, 60.0, 256, 2048, 0), (1 << 12, 2.0, 1024, 2048, 1),
+    (1 << 13, 8.0, 64, 2048, 1), (1 << 13, 8.0, 64, 2048, 0), (1 << 13, 60.0, 256, 2048, 0), (1 << 12, 2.0, 1024, 2048, 1), (1 << 13, 4.0, 256, 2048, 1),
 ])
 def test_correlate_all_modes(emu, N, zmax, m, L, ib):
     cfg = synth.small_config(N, zmax, 2.0, m, L, interbin=ib, index=20 + ib)
