@@ -125,7 +125,7 @@ def run_ours(args):
     import numpy as np
     import torch
     import torch.distributed as dist
-    from paper_1511_07343_b200 import build as fbuild, fdas, synth
+    from paper_1511_07343_b200 import build as fbuild, fdas, shard, synth
 
     rank = int(os.environ.get("RANK", "0"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
@@ -146,9 +146,10 @@ def run_ours(args):
     info = plan.info
     base = cfg.series()                         # seeded series with the 8 injected signals
     host = torch.empty((n_rot, cfg.n_samples), dtype=torch.float32).pin_memory()
-    for r in range(n_rot):                      # independent noise per DM (seed per DM and per rank), same signals
-        host[r] = torch.from_numpy(base if (r == 0 and rank == 0) else
-                                   synth.make_series(cfg.n_samples, cfg.series_seed(1 + r + n_rot * rank), cfg.signals[0]))
+    my_dms = shard.dm_shard(n_rot * world, rank, world)     # global DM-trial indices of this rank (dm mod world)
+    for r, dm in enumerate(my_dms):             # independent noise per DM trial (seed per DM), same 8 signals
+        host[r] = torch.from_numpy(base if dm == 0 else
+                                   synth.make_series(cfg.n_samples, cfg.series_seed(dm), cfg.signals[0]))
     d_series = host.cuda()
     d_spec = plan.empty_spectrum(1)
     d_mu = torch.empty(1, dtype=torch.float32, device="cuda")
@@ -190,17 +191,27 @@ def run_ours(args):
     stage = np.array([[m[j].elapsed_time(m[j + 1]) for j in range(3)] for m in marks]).mean(axis=0)
     n_found = int(cands[1][0])
 
-    # end to end through the host-buffer entry point (pinned host series in, candidate list out)
-    h_c = np.zeros((1, cap), dtype=fdas.CAND_DTYPE)
-    h_n = np.zeros(1, dtype=np.uint32)
-    plan.search_host(host[0:1], 16, thr, cap, h_c, h_n)          # warm-up: allocates the arena
-    e2e_steps = max(3, min(args.steps, 10))
+    # end to end through the host-buffer entry point: pinned host series in, candidate lists out.  One call
+    # searches a batch of n_e2e DM trials (the n_rot series, repeated) and overlaps the copy of series i+1
+    # with the kernels of series i inside the library (PAPER.md:49 step 1); every series is copied
+    # host->device and every candidate list device->host inside the timed region.
+    n_e2e = max(4, min(args.steps, 16))
+    host_e2e = torch.empty((n_e2e, cfg.n_samples), dtype=torch.float32).pin_memory()
+    for i in range(n_e2e):
+        host_e2e[i] = host[i % n_rot]
+    e2e_cap = 1 << 20
+    h_c = torch.zeros((n_e2e, e2e_cap, 3), dtype=torch.int32).pin_memory()
+    h_n = torch.zeros(n_e2e, dtype=torch.int32).pin_memory()
+    plan.search_host(host_e2e, 16, thr, e2e_cap, h_c, h_n)          # warm-up: allocates the arena, streams, events
     torch.cuda.synchronize()
+    e2e_rep = 2
     t0 = time.perf_counter()
-    for i in range(e2e_steps):
-        plan.search_host(host[i % n_rot:i % n_rot + 1], 16, thr, cap, h_c, h_n)
-    e2e_ms = (time.perf_counter() - t0) * 1e3 / e2e_steps
-    d2h = int(h_n[0]) * 12 + 4
+    for _ in range(e2e_rep):
+        plan.search_host(host_e2e, 16, thr, e2e_cap, h_c, h_n)
+    e2e_ms = (time.perf_counter() - t0) * 1e3 / (e2e_rep * n_e2e)
+    counts = h_n.numpy().astype(np.int64)
+    assert (counts <= e2e_cap).all() and counts.min() > 0, "e2e candidate lists overflowed or empty"
+    d2h = int(counts.mean()) * 12 + 4
     clocks = sampler.stop() if rank == 0 else None
 
     t = torch.tensor([ms, e2e_ms], dtype=torch.float64, device="cuda")
@@ -214,13 +225,42 @@ def run_ours(args):
     ms_step = ms / args.steps
     value = world * 1e3 / ms_step
     flops = workload_flops(info)
-    corr_ms = float(stage[1])
-    achieved = flops / (corr_ms * 1e-3) / 1e12
-    hbm_peak = None
+    spec_ms, corr_ms, hs_ms = (float(v) for v in stage)
+    peaks = {}
     try:
-        hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
     except Exception:
         pass
+    hbm_peak = peaks.get("hbm_gbs", 6650.0)
+    hbm_src = "MEASURED_PEAKS.json hbm_gbs (of measured)" if "hbm_gbs" in peaks else "6650 GB/s (of fallback, B200_PROFILING.md)"
+    plane_bytes = 4 * info.n_templates * info.n_bins
+    corr_tf = flops / (corr_ms * 1e-3) / 1e12
+    kernels = {
+        "spectrum": {"kernels": "k_spec_pass1 + k_spec_pass2", "bound": "hbm", "ms": spec_ms,
+                     "algorithmic_bytes": 4 * cfg.n_samples + 8 * info.n_bins,
+                     "achieved": (4 * cfg.n_samples + 8 * info.n_bins) / (spec_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s"},
+        "correlate": {"kernels": "k_correlate_2048_v2", "bound": "alu", "ms": corr_ms, "algorithmic_flops": flops,
+                      "achieved": corr_tf, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                      "hbm_side": {"bytes": plane_bytes + 8 * info.n_bins,
+                                   "achieved_gbs": (plane_bytes + 8 * info.n_bins) / (corr_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak}},
+        "harmsum": {"kernels": "k_harmsum<5,...>", "bound": "hbm", "ms": hs_ms, "algorithmic_bytes": plane_bytes,
+                    "achieved": plane_bytes / (hs_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s"},
+    }
+    for k in kernels.values():
+        k["frac"] = k["achieved"] / k["peak"]
+    dom = max(kernels, key=lambda n: kernels[n]["ms"])          # the kernel with the largest share of the step
+    kd = kernels[dom]
+    roofline = {"kernel": dom + " (" + kd["kernels"] + ")", "bound": kd["bound"], "achieved": kd["achieved"],
+                "peak": kd["peak"], "unit": kd["unit"], "frac": kd["frac"], "traffic": None,
+                "ms_per_launch": kd["ms"], "share_of_step": kd["ms"] / (spec_ms + corr_ms + hs_ms),
+                "peak_source": hbm_src if kd["bound"] == "hbm" else
+                "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
+                "per_unit": "bytes: the plane read once (4 n_t n_bins)" if dom == "harmsum" else
+                "flops: SURVEY 8(d) convention, bench.py::workload_flops" if dom == "correlate" else "bytes: series + spectrum"}
+    # north_star's FFT-correlation roofline for spectrum + correlate: the slower of flops at FP32 peak and bytes at HBM peak
+    fft_flops = flops + 2.5 * cfg.n_samples * math.log2(cfg.n_samples)
+    fft_bytes = 4 * cfg.n_samples + plane_bytes
+    t_roof_ms = max(fft_flops / (FP32_PEAK_TFLOPS * 1e12), fft_bytes / (hbm_peak * 1e9)) * 1e3
     out = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -232,20 +272,18 @@ def run_ours(args):
                                                   "per step: inputs exceed the 126 MB L2",
                    "parallelism": "DM trials sharded across ranks, no collective"},
         "plane_outputs_per_s": world * info.n_templates * info.n_bins / (corr_ms * 1e-3),
-        "stage_ms": {"spectrum": float(stage[0]), "correlate": corr_ms, "harmsum": float(stage[2])},
+        "stage_ms": {"spectrum": spec_ms, "correlate": corr_ms, "harmsum": hs_ms},
+        "fft_correlation_roofline": {"ms_at_roofline": t_roof_ms, "ms_measured": spec_ms + corr_ms,
+                                     "frac": t_roof_ms / (spec_ms + corr_ms),
+                                     "dm_trials_per_s_without_harmsum": world * 1e3 / (spec_ms + corr_ms)},
         "candidates_found": n_found,
         "gpu_launches": 4 * args.steps,
         "clocks": clocks,
         "e2e": {"value": world * 1e3 / e2e_ms, "unit": UNIT, "ms_per_step": e2e_ms,
-                "h2d_bytes_per_step": cfg.n_samples * 4, "d2h_bytes_per_step": d2h},
-        "roofline": {"kernel": "fused correlate (forward FFT, template multiply, inverse FFT, power, store)",
-                     "bound": "alu", "achieved": achieved, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / FP32_PEAK_TFLOPS, "traffic": None,
-                     "flops_per_launch": flops, "ms_per_launch": corr_ms,
-                     "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md)",
-                     "hbm_side": {"bytes_per_launch": 4 * info.n_templates * info.n_bins + 8 * info.n_bins,
-                                  "achieved_gbs": (4 * info.n_templates * info.n_bins + 8 * info.n_bins) / (corr_ms * 1e-3) / 1e9,
-                                  "peak_gbs": hbm_peak}},
+                "h2d_bytes_per_step": cfg.n_samples * 4, "d2h_bytes_per_step": d2h,
+                "how": "fdas_search_host on %d pinned series per call, x%d calls" % (n_e2e, e2e_rep)},
+        "roofline": roofline,
+        "kernels": kernels,
     }
     if world == 1 and not args.no_cpu:
         import oracle

@@ -148,7 +148,9 @@ def fdas_candidates(plan, d_plane, threshold, d_cands, d_count, capacity, stream
 
 def fdas_search_host(plan, h_series: np.ndarray, max_harm, thresholds, capacity, h_cands=None, h_counts=None,
                      stream=None):
-    """Host-buffer path: h_series float32[n_batch, N] (numpy or pinned torch CPU tensor)."""
+    """Host-buffer path: h_series float32[n_batch, N] (numpy, or a pinned torch CPU tensor for truly
+    asynchronous copies); h_cands [n_batch, capacity] 12-byte records and h_counts [n_batch] uint32, numpy
+    or pinned torch CPU tensors (int32[n_batch, capacity, 3] / int32[n_batch])."""
     if isinstance(h_series, torch.Tensor):
         ptr, n_batch = h_series.data_ptr(), (h_series.shape[0] if h_series.dim() == 2 else 1)
     else:
@@ -159,9 +161,10 @@ def fdas_search_host(plan, h_series: np.ndarray, max_harm, thresholds, capacity,
         h_cands = np.zeros((n_batch, capacity), dtype=CAND_DTYPE)
     if h_counts is None:
         h_counts = np.zeros(n_batch, dtype=np.uint32)
+    hptr = lambda a: C.c_void_p(a.data_ptr()) if isinstance(a, torch.Tensor) else a.ctypes.data_as(C.c_void_p)
     _check(lib().fdas_search_host(plan, C.c_void_p(ptr), int(n_batch), int(max_harm),
-                                  thr.ctypes.data_as(C.c_void_p), h_cands.ctypes.data_as(C.c_void_p),
-                                  h_counts.ctypes.data_as(C.c_void_p), int(capacity), _stream(stream)),
+                                  thr.ctypes.data_as(C.c_void_p), hptr(h_cands), hptr(h_counts), int(capacity),
+                                  _stream(stream)),
            "fdas_search_host")
     return h_cands, h_counts
 
