@@ -16,6 +16,10 @@
  *     never allocates in the d_* hot calls. The plan owns only the template bank and a
  *     few KB of metadata; fdas_search_host additionally owns a scratch arena it
  *     allocates on first use.
+ *   - Alignment of device pointers (FDAS_E_INVALID otherwise; what cudaMalloc and PyTorch return
+ *     always qualifies): d_series and d_spectrum 8 bytes, d_plane 16 bytes for fdas_correlate and
+ *     4 bytes for fdas_harmsum / fdas_candidates, candidate lists and counters 4 bytes, the
+ *     workspace 256 bytes.
  *   - `stream` is a cudaStream_t passed as void* (NULL = default stream). Every d_* hot
  *     call only enqueues work and returns; nothing synchronises.
  *   - Return value: FDAS_OK (0) or a negative FDAS_E_* code. No exceptions, no exit().

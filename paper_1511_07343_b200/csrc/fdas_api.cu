@@ -16,6 +16,9 @@ void fdas_set_cuda_error(cudaError_t e, const char* where)
 
 char* fdas_cuda_error_text() { return g_cuda_err; }
 
+// Vector accesses in the kernels need these alignments (a misaligned device pointer would fault on the GPU).
+static bool misaligned(const void* ptr, uintptr_t a) { return ((uintptr_t)ptr & (a - 1)) != 0; }
+
 static bool is_pow2(int64_t v) { return v > 0 && (v & (v - 1)) == 0; }
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -141,6 +144,7 @@ extern "C" int fdas_spectrum(fdas_plan* p, const float* d_series, int32_t n_batc
                              float* d_meanpow, void* d_workspace, void* stream)
 {
     if (!p || !d_series || !d_spectrum || n_batch < 1 || n_batch > p->max_batch) return FDAS_E_INVALID;
+    if (misaligned(d_series, 8) || misaligned(d_spectrum, 8) || misaligned(d_meanpow, 4)) return FDAS_E_INVALID;
     if (!d_workspace || ((uintptr_t)d_workspace & 255)) return FDAS_E_WORKSPACE;
     return fdas_launch_spectrum(p, d_series, n_batch, reinterpret_cast<float2*>(d_spectrum), d_meanpow,
                                 d_workspace, (cudaStream_t)stream);
@@ -154,6 +158,8 @@ extern "C" int fdas_correlate(fdas_plan* p, const float* d_spectrum, int32_t n_b
     if (!p || !d_spectrum || n_batch < 1) return FDAS_E_INVALID;
     if (!d_plane && !d_cands) return FDAS_E_INVALID;
     if (d_cands && !d_counts) return FDAS_E_INVALID;
+    if (misaligned(d_spectrum, 8) || misaligned(d_plane, 16) || misaligned(d_cands, 4) || misaligned(d_counts, 4))
+        return FDAS_E_INVALID;
     if (!p->built) return FDAS_E_STATE;
     return fdas_launch_correlate(p, reinterpret_cast<const float2*>(d_spectrum), n_batch, d_plane, threshold,
                                  d_cands, d_counts, capacity, (cudaStream_t)stream);
@@ -166,6 +172,7 @@ extern "C" int fdas_harmsum(fdas_plan* p, const float* d_plane, int32_t max_harm
 {
     if (!p || !d_plane || !h_thresholds || !d_cands || !d_count) return FDAS_E_INVALID;
     if (!valid_max_harm(max_harm) || p->interbin) return FDAS_E_INVALID;
+    if (misaligned(d_plane, 4) || misaligned(d_cands, 4) || misaligned(d_count, 4)) return FDAS_E_INVALID;
     return fdas_launch_harmsum(p, d_plane, max_harm, h_thresholds, d_cands, d_count, capacity, (cudaStream_t)stream);
 }
 
@@ -173,5 +180,6 @@ extern "C" int fdas_candidates(fdas_plan* p, const float* d_plane, float thresho
                                uint32_t* d_count, uint32_t capacity, void* stream)
 {
     if (!p || !d_plane || !d_cands || !d_count) return FDAS_E_INVALID;
+    if (misaligned(d_plane, 4) || misaligned(d_cands, 4) || misaligned(d_count, 4)) return FDAS_E_INVALID;
     return fdas_launch_candidates(p, d_plane, threshold, d_cands, d_count, capacity, (cudaStream_t)stream);
 }

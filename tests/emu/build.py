@@ -46,13 +46,14 @@ def build(force: bool = False) -> str:
     for u in units:
         o = os.path.join(OUT, os.path.basename(u)[:-4] + ".o")
         objs.append(o)
-        cmd = ["g++", "-std=c++17", "-O2", "-g", "-fPIC", "-fno-strict-aliasing", "-I", HERE, "-c", u, "-o", o]
+        cmd = ["g++", "-std=c++17", "-O2", "-g", "-fPIC", "-fno-strict-aliasing", "-fsanitize=alignment",
+               "-fno-sanitize-recover=alignment", "-I", HERE, "-c", u, "-o", o]
         procs.append((u, subprocess.Popen(cmd, stdout=subprocess.PIPE, stderr=subprocess.STDOUT, text=True)))
     for u, p in procs:
         out, _ = p.communicate()
         if p.returncode:
             raise RuntimeError("g++ failed on %s:\n%s" % (u, out))
-    subprocess.check_call(["g++", "-shared", "-o", LIB, *objs, "-lpthread"])
+    subprocess.check_call(["g++", "-shared", "-fsanitize=alignment", "-o", LIB, *objs, "-lpthread"])
     return LIB
 
 

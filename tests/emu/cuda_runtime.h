@@ -17,9 +17,9 @@
 #define __shared__ thread_local
 #define __align__(n) __attribute__((aligned(n)))
 
-struct float2 { float x, y; };
+struct alignas(8) float2 { float x, y; };          // CUDA's alignments: the emu build runs with -fsanitize=alignment
 struct alignas(16) float4 { float x, y, z, w; };
-struct double2 { double x, y; };
+struct alignas(16) double2 { double x, y; };
 struct uint3 { unsigned x, y, z; };
 struct dim3 {
     unsigned x, y, z;

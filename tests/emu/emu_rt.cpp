@@ -20,7 +20,7 @@ static std::mutex g_mu;
 static const size_t PG = 4096;
 static bool align_end() { const char* e = getenv("EMU_ALIGN"); return !(e && !strcmp(e, "start")); }
 
-static void* guarded_alloc(size_t n)
+static void* guarded_alloc(size_t n, bool poison = true)
 {
     size_t body = (n + PG - 1) / PG * PG;
     if (body == 0) body = PG;
@@ -31,7 +31,7 @@ static void* guarded_alloc(size_t n)
     mprotect(m + PG + body, PG, PROT_NONE);
     char* user = m + PG;
     if (align_end()) user = m + PG + body - ((n + 15) / 16 * 16);
-    memset(m + PG, 0xA5, body);                  // poison: uninitialised reads give garbage, like the GPU
+    if (poison) memset(m + PG, 0xFF, body);                  // poison: an uninitialised float reads as NaN and shows up in parity
     std::lock_guard<std::mutex> lk(g_mu);
     g_allocs[(uintptr_t)user] = Alloc{m, len, user, n};
     return user;
@@ -92,10 +92,41 @@ __attribute__((constructor)) static void install()
 
 // ------------------------------------------------------------------ CTA scheduler
 enum { ST_RUN = 0, ST_BLOCK_BAR = 1, ST_WARP_BAR = 2, ST_DONE = 3 };
-struct Fiber { ucontext_t ctx; char* stack; int state; uint3 tid; };
+#if defined(__x86_64__)
+// Minimal user-level context switch (callee-saved registers + stack pointer): swapcontext makes a
+// signal-mask system call per switch, which dominates the run time of barrier-heavy kernels.
+extern "C" void emu_switch(void** save_sp, void* load_sp);
+asm(".text\n.globl emu_switch\n.type emu_switch,@function\nemu_switch:\n"
+    "  pushq %rbp\n  pushq %rbx\n  pushq %r12\n  pushq %r13\n  pushq %r14\n  pushq %r15\n"
+    "  movq %rsp, (%rdi)\n  movq %rsi, %rsp\n"
+    "  popq %r15\n  popq %r14\n  popq %r13\n  popq %r12\n  popq %rbx\n  popq %rbp\n  ret\n"
+    ".size emu_switch, .-emu_switch\n");
+struct Ctx { void* sp; };
+static void ctx_switch(Ctx* from, Ctx* to) { emu_switch(&from->sp, to->sp); }
+static void ctx_make(Ctx* c, char* stack, size_t size, void (*fn)(), Ctx*)
+{
+    uintptr_t top = ((uintptr_t)stack + size) & ~(uintptr_t)15;
+    void** sp = (void**)(top - 16);              // return address slot, 16-byte aligned: fn enters with rsp % 16 == 8
+    *sp = (void*)fn;
+    for (int i = 0; i < 6; i++) *--sp = nullptr; // rbp rbx r12 r13 r14 r15
+    c->sp = sp;
+}
+#else
+struct Ctx { ucontext_t uc; };
+static void ctx_switch(Ctx* from, Ctx* to) { swapcontext(&from->uc, &to->uc); }
+static void ctx_make(Ctx* c, char* stack, size_t size, void (*fn)(), Ctx* link)
+{
+    getcontext(&c->uc);
+    c->uc.uc_stack.ss_sp = stack;
+    c->uc.uc_stack.ss_size = size;
+    c->uc.uc_link = &link->uc;
+    makecontext(&c->uc, fn, 0);
+}
+#endif
+struct Fiber { Ctx ctx; char* stack; int state; uint3 tid; };
 struct Worker {
     std::vector<Fiber> fibers;
-    ucontext_t sched;
+    Ctx sched;
     int cur;
     const std::function<void()>* body;
     void* dyn_smem;
@@ -109,13 +140,14 @@ static void tramp()
     (*w->body)();
     w = t_w;
     w->fibers[w->cur].state = ST_DONE;
-    swapcontext(&w->fibers[w->cur].ctx, &w->sched);
+    ctx_switch(&w->fibers[w->cur].ctx, &w->sched);
+    abort();                                     // a finished fibre is never resumed
 }
 static void yield_with(int st)
 {
     Worker* w = t_w;
     w->fibers[w->cur].state = st;
-    swapcontext(&w->fibers[w->cur].ctx, &w->sched);
+    ctx_switch(&w->fibers[w->cur].ctx, &w->sched);
 }
 void emu_syncthreads() { yield_with(ST_BLOCK_BAR); }
 void emu_syncwarp() { yield_with(ST_WARP_BAR); }
@@ -127,15 +159,11 @@ static void run_block(Worker* w, dim3 block, bool rev)
     if ((int)w->fibers.size() < nt) {
         size_t old = w->fibers.size();
         w->fibers.resize(nt);
-        for (size_t i = old; i < (size_t)nt; i++) w->fibers[i].stack = (char*)guarded_alloc(STACK);
+        for (size_t i = old; i < (size_t)nt; i++) w->fibers[i].stack = (char*)guarded_alloc(STACK, false);
     }
     for (int i = 0; i < nt; i++) {
         Fiber& f = w->fibers[i];
-        getcontext(&f.ctx);
-        f.ctx.uc_stack.ss_sp = f.stack;
-        f.ctx.uc_stack.ss_size = STACK;
-        f.ctx.uc_link = &w->sched;
-        makecontext(&f.ctx, tramp, 0);
+        ctx_make(&f.ctx, f.stack, STACK, tramp, &w->sched);
         f.state = ST_RUN;
         f.tid = uint3{(unsigned)i % block.x, ((unsigned)i / block.x) % block.y, (unsigned)i / (block.x * block.y)};
     }
@@ -148,7 +176,7 @@ static void run_block(Worker* w, dim3 block, bool rev)
             if (f.state != ST_RUN) continue;
             w->cur = i;
             threadIdx = f.tid;
-            swapcontext(&w->sched, &f.ctx);
+            ctx_switch(&w->sched, &f.ctx);
             progress = true;
             if (f.state == ST_DONE) done++;
         }

@@ -85,6 +85,13 @@ def test_state_and_argument_errors_without_gpu(fdas):
     assert lib.fdas_spectrum(h, one, 1, one, None, None, None) == fdas.FDAS_E_WORKSPACE
     assert lib.fdas_spectrum(h, one, 1, one, None, C.c_void_p(8), None) == fdas.FDAS_E_WORKSPACE
     assert lib.fdas_spectrum(h, one, 2, one, None, one, None) == fdas.FDAS_E_INVALID      # n_batch > MAX_BATCH
+    # misaligned device pointers are refused before anything is launched (include/fdas.h, Conventions)
+    odd4, odd8 = C.c_void_p(260), C.c_void_p(264)
+    assert lib.fdas_spectrum(h, odd4, 1, one, None, one, None) == fdas.FDAS_E_INVALID
+    assert lib.fdas_spectrum(h, one, 1, odd4, None, one, None) == fdas.FDAS_E_INVALID
+    assert lib.fdas_correlate(h, odd4, 1, one, 0.0, None, None, 0, None, None) == fdas.FDAS_E_INVALID
+    assert lib.fdas_correlate(h, one, 1, odd8, 0.0, None, None, 0, None, None) == fdas.FDAS_E_INVALID
+    assert lib.fdas_candidates(h, C.c_void_p(258), 1.0, one, one, 1, None) == fdas.FDAS_E_INVALID
     thr = np.ones(5, np.float32)
     assert lib.fdas_harmsum(h, one, 3, thr.ctypes.data_as(C.c_void_p), one, one, 1, None) == fdas.FDAS_E_INVALID
     assert b"invalid" in lib.fdas_strerror(fdas.FDAS_E_INVALID)
