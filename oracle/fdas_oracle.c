@@ -26,8 +26,9 @@
  *                        nearest grid point, integer-exact rounding       [O6]
  *   ofdas_threshold      Q(H, T) = e^-T sum_{j<H} T^j/j! = pfa (chi^2, 2H dof)
  *
- * Pins: tests/test_oracle_pins.py (P1..P12 of DESIGN.md).  Parity unpinned:
- * harmonic-sum behaviour on real multi-harmonic pulsar signals (paper silent).
+ * Pins: tests/test_oracle_pins.py (P1..P13 of DESIGN.md).  The harmonic sum is pinned by its
+ * index rule (P12) and by the closed form for a noise-free pulse train (P13); its statistics
+ * on real pulsar data are outside what the paper fixes (paper silent) and stay unpinned.
  */
 #include <complex.h>
 #include <math.h>

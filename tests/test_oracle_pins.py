@@ -340,3 +340,35 @@ def test_harmsum_stage_nesting_identity():
     _, S = oracle.harmsum(P, 8, np.full(4, 1e9), return_sums=True)
     assert np.all(S[1] >= S[0]) and np.all(S[2] >= S[1]) and np.all(S[3] >= S[2])
     assert np.allclose(S[0], P)
+
+
+def test_P13_harmsum_of_a_noise_free_pulse_train():
+    """End-to-end pin of the harmonic-sum reading G16: (k, zeta) label the TOP
+    harmonic, and both the bin and the z index are stretched by h/H.  A noise-free train with harmonics
+    h = 1..4 of a fundamental at bin r0 = 300 drifting z0 = 2 bins puts its h-th harmonic at (h r0, h z0)
+    ("pulse harmonics", z scales with the frequency).  By P6 the plane peaks there
+    at (A_h N/2)^2 / mu, so the closed form is
+        S_H(H r0, H z0) = sum_{h<=H} (A_h N/2)^2 / mu,
+    it is the global maximum of stage H, and the fundamental-labelled reading (sums placed at (r0, z0))
+    finds only the h = 1 peak."""
+    N, r0, z0 = 1 << 14, 300, 2
+    amps = [1.0, 0.8, 0.6, 0.5]
+    sig = [synth.Signal(a, r0 * (h + 1), z0 * (h + 1), 0.3 * h) for h, a in enumerate(amps)]
+    x = synth.make_series(N, 1, sig, noise=False)
+    S, mu = oracle.spectrum(x)
+    T = oracle.templates(8.0, 2.0, 64)
+    P = oracle.correlate_fft(S, T, 1024)
+    peak = [(a * N / 2) ** 2 / mu for a in amps]
+    zi = lambda z: int((z + 8) // 2)
+    for h in range(4):                                           # P6 at each harmonic: the plane itself
+        assert P[zi(z0 * (h + 1)), r0 * (h + 1) - 1] == pytest.approx(peak[h], rel=2e-3)
+    thr = np.array([1e30, 1e30, 1e30])
+    _, sums = oracle.harmsum(P, 4, thr, bin0=1, return_sums=True)
+    for st, H in enumerate((1, 2, 4)):
+        want = sum(peak[:H])
+        got = sums[st][zi(z0 * H), r0 * H - 1]
+        assert got == pytest.approx(want, rel=2e-3), (H, got, want)
+        if H > 1:
+            assert np.unravel_index(np.argmax(sums[st]), sums[st].shape) == (zi(z0 * H), r0 * H - 1)
+    # fundamental labelling would look at (r0, z0) and see one harmonic only
+    assert sums[2][zi(z0), r0 - 1] < 1.05 * peak[0]
