@@ -123,7 +123,8 @@ void ofdas_dft_direct(const cplx *x, cplx *out, int64_t n, int sign)
 /* O1.  x: float32[N] widened to double.  F = DFT_N(x) (forward, unnormalised);
  * keep k = 1..N/2 (drop DC, keep Nyquist): S[c] = F[c+1]/sqrt(mu),
  * mu = mean_{k=1..N/2} |F_k|^2.   F_raw (optional, N/2+1 entries k=0..N/2) gets
- * the un-normalised bins for the Parseval pin. */
+ * the un-normalised bins for the Parseval pin.  Degenerate case (paper silent; DESIGN.md
+ * reading G22): a series whose kept bins are all exactly zero has mu = 0 and S := 0. */
 int ofdas_spectrum(const float *x, int64_t N, cplx *S, double *mu_out, cplx *F_raw)
 {
     if (N < 4 || (N & (N - 1))) return -1;
@@ -136,7 +137,7 @@ int ofdas_spectrum(const float *x, int64_t N, cplx *S, double *mu_out, cplx *F_r
     double acc = 0.0;
     for (int64_t k = 1; k <= nb; k++) acc += creal(a[k]) * creal(a[k]) + cimag(a[k]) * cimag(a[k]);
     double mu = acc / (double)nb;
-    double s = 1.0 / sqrt(mu);
+    double s = mu > 0.0 ? 1.0 / sqrt(mu) : 0.0;
     for (int64_t c = 0; c < nb; c++) S[c] = a[c + 1] * s;
     if (F_raw) for (int64_t k = 0; k <= nb; k++) F_raw[k] = a[k];
     if (mu_out) *mu_out = mu;

@@ -81,7 +81,7 @@ k_spec_pass2(const float2* __restrict__ inter, const double* __restrict__ part, 
         double N = 2.0 * (double)M;
         double tot = 0.5 * (N * red[1][0] - red[0][0] * red[0][0] + red[2][0] * red[2][0]);
         double mu = tot / (double)M;
-        s_scale = (float)(1.0 / sqrt(mu));
+        s_scale = mu > 0.0 ? (float)(1.0 / sqrt(mu)) : 0.0f;      // all-zero series: S := 0 (G22)
         if (meanpow && blockIdx.x == 0) meanpow[bt] = (float)mu;
     }
     // load rows

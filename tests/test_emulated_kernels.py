@@ -64,6 +64,19 @@ def test_spectrum(emu, log2n):
     plan.close()
 
 
+def test_all_zero_series(emu):
+    """Degenerate input (G22): zero spectrum, zero plane, no candidates, nothing NaN."""
+    N = 1 << 13
+    plan = emu.Plan(N, 4.0, 2.0, 64, 2048, quad_points=256)
+    d_S, d_mu = plan.spectrum(np.zeros(N, np.float32))
+    assert float(d_mu.np()[0]) == 0.0 and not np.any(d_S.np())
+    d_P, _, d_n = plan.correlate(d_S, True, 0.5, 16)
+    assert not np.any(d_P.np()) and int(d_n.np()[0]) == 0
+    c, n = plan.harmsum(d_P, 16, oracle.thresholds(16), 16)
+    assert n == 0
+    plan.close()
+
+
 def test_spectrum_batched(emu):
     N = 1 << 12
     xs = np.stack([synth.make_series(N, 900 + b) * (1.0 + b) for b in range(3)])

@@ -98,6 +98,21 @@ def test_spectrum_batched(fdas):
         assert float(d_mu[b]) == pytest.approx(mu, rel=2e-6)
 
 
+def test_all_zero_series(fdas):
+    """Degenerate input (G22): zero spectrum, zero plane, no candidates, nothing NaN."""
+    N = 1 << 13
+    plan = fdas.Plan(N, 4.0, 2.0, 64, 2048)
+    d_S, d_mu = plan.spectrum(torch.zeros((1, N), device="cuda"))
+    assert float(d_mu[0]) == 0.0 and not bool(d_S.any())
+    d_P = plan.empty_plane(1)
+    cands = plan.empty_cands(16)
+    plan.correlate(d_S, d_P, threshold=0.5, cands=cands, capacity=16)
+    assert not bool(d_P.any()) and int(cands[1][0]) == 0
+    hs = plan.empty_cands(16)
+    plan.harmsum(d_P[0], 16, fdas.thresholds(16), hs, 16)
+    assert int(hs[1][0]) == 0
+
+
 # ------------------------------------------------------------------ correlate (rows a2-a6)
 def run_gpu_plane(fdas, plan, x, thr=None, cap=1 << 16):
     d_x = torch.from_numpy(np.ascontiguousarray(x)).cuda().view(1, -1)

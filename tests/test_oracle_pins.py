@@ -372,3 +372,9 @@ def test_P13_harmsum_of_a_noise_free_pulse_train():
             assert np.unravel_index(np.argmax(sums[st]), sums[st].shape) == (zi(z0 * H), r0 * H - 1)
     # fundamental labelling would look at (r0, z0) and see one harmonic only
     assert sums[2][zi(z0), r0 - 1] < 1.05 * peak[0]
+
+
+def test_all_zero_series_gives_zero_spectrum_G22():
+    """Degenerate input (reading G22): mu = 0 -> S := 0, not 0/0."""
+    S, mu = oracle.spectrum(np.zeros(1 << 10, np.float32))
+    assert mu == 0.0 and not np.any(S)
