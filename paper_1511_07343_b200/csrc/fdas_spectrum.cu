@@ -12,8 +12,12 @@
 #include "fdas_common.cuh"
 #include "fdas_smemfft.cuh"
 
-// pass 1: grid = (R2/C, n_batch), block 256, smem 2*C*(R1+1) float2.
-__global__ void __launch_bounds__(256)
+// threads per CTA of both passes: the 131 KB tiles allow one CTA per SM, so the CTA itself must carry
+// enough warps (16) to keep loads in flight while others compute
+constexpr int SPEC_THREADS = 512;
+
+// pass 1: grid = (R2/C, n_batch), block SPEC_THREADS, smem 2*C*(R1+1) float2.
+__global__ void __launch_bounds__(SPEC_THREADS)
 k_spec_pass1(const float* __restrict__ series, float2* __restrict__ inter, double* __restrict__ part,
              int M, int R1, int R2, int C)
 {
@@ -42,10 +46,10 @@ k_spec_pass1(const float* __restrict__ series, float2* __restrict__ inter, doubl
         inter[(size_t)bt * M + (size_t)k1 * R2 + n2] = v;
     }
     // block reduction of the three sums (fixed tree)
-    __shared__ double red[3][256];
+    __shared__ double red[3][SPEC_THREADS];
     red[0][threadIdx.x] = s1; red[1][threadIdx.x] = s2; red[2][threadIdx.x] = sa;
     __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
+    for (int o = SPEC_THREADS / 2; o > 0; o >>= 1) {
         if (threadIdx.x < o)
             for (int q = 0; q < 3; q++) red[q][threadIdx.x] += red[q][threadIdx.x + o];
         __syncthreads();
@@ -53,14 +57,14 @@ k_spec_pass1(const float* __restrict__ series, float2* __restrict__ inter, doubl
     if (threadIdx.x < 3) part[((size_t)bt * gridDim.x + blockIdx.x) * 3 + threadIdx.x] = red[threadIdx.x][0];
 }
 
-// pass 2: grid = (ceil((R1/2+1)/C), n_batch), block 256, smem 2*(2C)*(R2+1) float2.
+// pass 2: grid = (ceil((R1/2+1)/C), n_batch), block SPEC_THREADS, smem 2*(2C)*(R2+1) float2.
 // Rows [0,C): k1 = g*C + i ("low"), rows [C,2C): the mirrors (R1 - k1) mod R1.
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(SPEC_THREADS)
 k_spec_pass2(const float2* __restrict__ inter, const double* __restrict__ part, int n_part,
              float2* __restrict__ spec, float* __restrict__ meanpow, int M, int R1, int R2, int C)
 {
     extern __shared__ float2 sm[];
-    __shared__ double red[3][256];
+    __shared__ double red[3][SPEC_THREADS];
     __shared__ float s_scale;
     const int pitch = R2 + 1;
     float2* a = sm;
@@ -72,7 +76,7 @@ k_spec_pass2(const float2* __restrict__ inter, const double* __restrict__ part, 
         for (int q = 0; q < 3; q++) acc[q] += part[((size_t)bt * n_part + i) * 3 + q];
     for (int q = 0; q < 3; q++) red[q][threadIdx.x] = acc[q];
     __syncthreads();
-    for (int o = 128; o > 0; o >>= 1) {
+    for (int o = SPEC_THREADS / 2; o > 0; o >>= 1) {
         if (threadIdx.x < o)
             for (int q = 0; q < 3; q++) red[q][threadIdx.x] += red[q][threadIdx.x + o];
         __syncthreads();
@@ -130,10 +134,10 @@ int fdas_launch_spectrum(fdas_plan* p, const float* d_series, int n_batch, float
     size_t sm2 = 2 * (size_t)(2 * p->C2) * (p->R2 + 1) * sizeof(float2);
     FDAS_CUDA(cudaFuncSetAttribute(k_spec_pass1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm1));
     FDAS_CUDA(cudaFuncSetAttribute(k_spec_pass2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm2));
-    k_spec_pass1<<<dim3(p->R2 / p->C1, n_batch), 256, sm1, st>>>(d_series, inter, part, p->M, p->R1, p->R2, p->C1);
+    k_spec_pass1<<<dim3(p->R2 / p->C1, n_batch), SPEC_THREADS, sm1, st>>>(d_series, inter, part, p->M, p->R1, p->R2, p->C1);
     FDAS_LAUNCH_CHECK();
     int g2 = (p->R1 / 2 + 1 + p->C2 - 1) / p->C2;
-    k_spec_pass2<<<dim3(g2, n_batch), 256, sm2, st>>>(inter, part, p->n_part, d_spec, d_meanpow,
+    k_spec_pass2<<<dim3(g2, n_batch), SPEC_THREADS, sm2, st>>>(inter, part, p->n_part, d_spec, d_meanpow,
                                                       p->M, p->R1, p->R2, p->C2);
     FDAS_LAUNCH_CHECK();
     return FDAS_OK;
