@@ -121,6 +121,46 @@ def run_reference(args):
     }))
 
 
+def run_sweep(args):
+    """--sweep-templates: the paper's one experiment (Fig. 2), execution time against the
+    number of templates for one 2^23-sample series: spectrum + fused correlate with the plane stored, for
+    21 ... 121 templates (z_max = n_t - 1, dz = 2, width 256, segment 2048).  One JSON line."""
+    import torch
+    from paper_1511_07343_b200 import build as fbuild, fdas, synth
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    fbuild.build()
+    cfg = synth.config(2)
+    d_x = torch.from_numpy(cfg.series()).cuda().view(1, -1)
+    stream = torch.cuda.current_stream()
+    rows = []
+    for n_t in (21, 41, 61, 85, 101, 121):
+        plan = fdas.Plan(cfg.n_samples, float(n_t - 1), 2.0, cfg.width, cfg.seg_len)
+        d_spec, d_mu, d_plane = plan.empty_spectrum(1), torch.empty(1, device="cuda"), plan.empty_plane(1)
+
+        def step():
+            fdas.fdas_spectrum(plan.handle, d_x, 1, d_spec, d_mu, plan.workspace)
+            fdas.fdas_correlate(plan.handle, d_spec, 1, d_plane, 0.0, None, None, 0)
+        for _ in range(max(3, args.warmup)):
+            step()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(args.steps):
+            step()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / args.steps
+        rows.append({"n_templates": n_t, "ms_per_dm": ms, "dm_trials_per_s": 1e3 / ms,
+                     "plane_outputs_per_s": n_t * plan.info.n_bins / (ms * 1e-3),
+                     "frac_of_fft_roofline": (workload_flops(plan.info) + 2.5 * cfg.n_samples * math.log2(cfg.n_samples))
+                     / (FP32_PEAK_TFLOPS * 1e12) / (ms * 1e-3)})
+        plan.close()
+        del d_plane
+    print(json.dumps({"sweep_templates": rows, "n_samples": cfg.n_samples, "width": cfg.width,
+                      "segment_len": cfg.seg_len, "steps": args.steps, "data": "synthetic",
+                      "note": "the plane (n_t x 2^22 fp32) is written every step: larger than L2 from 8 templates on"}))
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -304,9 +344,13 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--sweep-templates", action="store_true",
+                    help="time spectrum + correlate against the number of templates (PAPER.md Fig. 2) instead")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    if args.impl == "reference":
+    if args.sweep_templates:
+        run_sweep(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
