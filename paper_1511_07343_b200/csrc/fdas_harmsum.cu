@@ -27,14 +27,14 @@ __device__ __noinline__ void push_cand_hs(fdas_cand* list, uint32_t* count, uint
 template <int NST, int HS_CPT, bool CHECK>
 __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fdas_cand* __restrict__ cands,
                                              uint32_t* __restrict__ count, uint32_t cap, const HarmThr& thr,
-                                             int n_cols, int n_z, int bin0)
+                                             int n_cols, int n_z, int bin0, int tile, int zi_lo, int zi_hi)
 {
     constexpr int HS_COLS = 32 * HS_CPT;
-    const int col0 = blockIdx.x * HS_COLS + threadIdx.x;
+    const int col0 = tile * HS_COLS + threadIdx.x;
     const int zc = (n_z - 1) / 2;
     const int k = bin0 + col0;
     constexpr int HMAX = 1 << (NST - 1);
-    for (int zi = threadIdx.y; zi < n_z; zi += HS_ROWS_PER_PASS) {
+    for (int zi = zi_lo + threadIdx.y; zi < zi_hi; zi += blockDim.y) {
         const int zeta = zi - zc, az = abs(zeta), sg = zeta < 0 ? -1 : 1;
         // issue every gather of the row's HS_CPT cells first (all independent), then sum in stage order
         float v[HS_CPT][HMAX];
@@ -74,15 +74,85 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
     }
 }
 
+// Tile order.  The stretch (k, zeta) -> (k h/H, zeta h/H) moves a cell along the ray through the origin of
+// the (k, zeta) plane, so the 16 cells that read one source cell all lie on that ray, at k = x H/h: with the
+// plain order (all rows of a column tile together, columns ascending) they are 1/16 ... 15/16 of the plane
+// apart in time and nothing is left in L2 (7.4 GB of DRAM reads for a 1.43 GB plane in an ncu capture; an LRU
+// model of this order gives 7.36 GB).  The plane is therefore cut into S angular SECTORS of equal area that
+// are swept one after the other, columns ascending inside each.  Boundary ray j = 0..S is named by where it
+// leaves the rectangle [0, K] x [-n_z/2, n_z/2], u_j = -2 + 4 j/S:  |u| <= 1: through the far edge k = K at
+// row (n_z/2) u;  1 < |u| <= 2: through the top/bottom edge at column K (2 - |u|)  (|u| = 2: vertical).
+// Sector s holds, in the column tile whose last bin is kc, the rows ceil(zb_s(kc)) <= zeta < ceil(zb_{s+1}(kc))
+// -- a partition of the rows of every tile.  A sector is thin, so the span of plane that streams through L2
+// between two uses of a source cell fits (the same model: 1.54 GB at S = 16, 1.43-1.51 GB at S = 32 for a
+// 90-60 MB cache: the plane is read from DRAM about once).  S = 1 is the plain order; results do not depend on S.
+constexpr int HS_MAX_SECTORS = 64;
+constexpr int HS_TILES_PER_CTA = 8;      // consecutive column tiles of its sector per CTA (a sector is only a few rows thin)
+struct HarmSectors {
+    int n_sec;
+    int first_cta[HS_MAX_SECTORS + 1];       // sector s owns CTAs [first_cta[s], first_cta[s+1]), HS_TILES_PER_CTA column tiles each
+};
+
+__host__ __device__ inline double sector_boundary(int j, int S, double kc, double K, double zhalf)
+{
+    const double u = -2.0 + 4.0 * (double)j / (double)S, au = u < 0.0 ? -u : u;
+    if (au <= 1.0) return zhalf * u * kc / K;
+    const double c = K * (2.0 - au);
+    const double r = (c <= 0.0 || kc >= c) ? 1.0 : kc / c;
+    return u < 0.0 ? -zhalf * r : zhalf * r;
+}
+
 template <int NST, int HS_CPT, int MINB>
 __global__ void __launch_bounds__(256, MINB)
 k_harmsum(const float* __restrict__ plane, fdas_cand* __restrict__ cands, uint32_t* __restrict__ count,
-          uint32_t cap, HarmThr thr, int n_cols, int n_z, int bin0)
+          uint32_t cap, HarmThr thr, HarmSectors sec, int n_cols, int n_z, int bin0)
 {
     constexpr int HS_COLS = 32 * HS_CPT;
-    const bool edge = blockIdx.x == 0 || blockIdx.x * HS_COLS + HS_COLS > n_cols;     // CTA-uniform
-    if (edge) harmsum_tile<NST, HS_CPT, true>(plane, cands, count, cap, thr, n_cols, n_z, bin0);
-    else harmsum_tile<NST, HS_CPT, false>(plane, cands, count, cap, thr, n_cols, n_z, bin0);
+    int s = 0;
+    while (s + 1 < sec.n_sec && (int)blockIdx.x >= sec.first_cta[s + 1]) s++;      // CTA-uniform, <= 63 steps
+    const int n_tiles = (n_cols + HS_COLS - 1) / HS_COLS;
+    const int tile0 = (blockIdx.x - sec.first_cta[s]) * HS_TILES_PER_CTA;
+    const int zc = (n_z - 1) / 2;
+    const double K = (double)(bin0 + n_cols - 1), zhalf = 0.5 * (double)n_z;
+#pragma unroll 1
+    for (int tile = tile0; tile < min(n_tiles, tile0 + HS_TILES_PER_CTA); tile++) {
+        int zi_lo = 0, zi_hi = n_z;
+        if (sec.n_sec > 1) {
+            const double kc = (double)bin0 + (double)min(n_cols, (tile + 1) * HS_COLS) - 1.0;
+            zi_lo = max(0, min(n_z, (int)ceil(sector_boundary(s, sec.n_sec, kc, K, zhalf)) + zc));
+            zi_hi = max(0, min(n_z, (int)ceil(sector_boundary(s + 1, sec.n_sec, kc, K, zhalf)) + zc));
+            if (zi_lo >= zi_hi) continue;                                          // CTA-uniform
+        }
+        const bool edge = tile == 0 || tile * HS_COLS + HS_COLS > n_cols;          // CTA-uniform
+        if (edge) harmsum_tile<NST, HS_CPT, true>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi);
+        else harmsum_tile<NST, HS_CPT, false>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi);
+    }
+}
+
+// Sector -> CTA ranges.  A sector whose two boundary rays both leave through the top/bottom edge is empty
+// beyond the column where the shallower one leaves; only the tiles before that are launched.
+static HarmSectors make_sectors(int n_sec, int n_cols, int bin0, int cols_per_tile)
+{
+    HarmSectors hs;
+    hs.n_sec = n_sec;
+    const int n_tiles = (n_cols + cols_per_tile - 1) / cols_per_tile;
+    const double K = (double)(bin0 + n_cols - 1);
+    hs.first_cta[0] = 0;
+    for (int s = 0; s < n_sec; s++) {
+        int nt = n_tiles;
+        if (n_sec > 1) {
+            double u0 = fabs(-2.0 + 4.0 * s / n_sec), u1 = fabs(-2.0 + 4.0 * (s + 1) / n_sec);
+            double umin = u0 < u1 ? u0 : u1;
+            bool same_side = (-2.0 + 4.0 * s / n_sec) * (-2.0 + 4.0 * (s + 1) / n_sec) > 0.0;
+            if (same_side && umin > 1.0) {
+                double c_outer = K * (2.0 - umin);
+                long long t = (long long)(c_outer / cols_per_tile) + 2;
+                if (t < nt) nt = (int)t;
+            }
+        }
+        hs.first_cta[s + 1] = hs.first_cta[s] + (nt + HS_TILES_PER_CTA - 1) / HS_TILES_PER_CTA;
+    }
+    return hs;
 }
 
 // Threshold + compaction over one plane (row a8). grid-stride over float4 groups of a row.
@@ -119,21 +189,33 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     FDAS_CUDA(cudaMemsetAsync(d_count, 0, sizeof(uint32_t), st));
     int n_cols = (int)p->n_cols;
     static const int variant = getenv("FDAS_HS_VARIANT") ? atoi(getenv("FDAS_HS_VARIANT")) : 0;
-    dim3 block(32, HS_ROWS_PER_PASS);
-#define FDAS_HS_ARGS d_plane, d_cands, d_count, cap, thr, n_cols, p->n_z, p->bin0
-#define FDAS_HS_GRID(CPT) dim3((n_cols + 32 * CPT - 1) / (32 * CPT))
+    // sectors of the tile order (see k_harmsum): 16 by default, thin enough for the reuse distance to fit in
+    // L2, thick enough (~10 rows at the far end) for L1 to keep serving the row-direction reuse inside a stream
+    static const int env_sectors = getenv("FDAS_HS_SECTORS") ? atoi(getenv("FDAS_HS_SECTORS")) : 16;
+    static const int env_rows = getenv("FDAS_HS_ROWS") ? atoi(getenv("FDAS_HS_ROWS")) : 0;
+    int n_sec = env_sectors < 1 ? 1 : env_sectors;
+    if (n_sec > HS_MAX_SECTORS) n_sec = HS_MAX_SECTORS;
+    int rows = env_rows > 0 ? env_rows : (n_sec == 1 ? HS_ROWS_PER_PASS : 4);      // warps per CTA, one row each per pass
+    if (rows > HS_ROWS_PER_PASS) rows = HS_ROWS_PER_PASS;
+    dim3 block(32, rows);
+    HarmSectors sec;
+#define FDAS_HS_LAUNCH(NST, CPT, MINB)                                                              \
+    do {                                                                                            \
+        sec = make_sectors(n_sec, n_cols, p->bin0, 32 * CPT);                                       \
+        k_harmsum<NST, CPT, MINB><<<dim3(sec.first_cta[n_sec]), block, 0, st>>>(                    \
+            d_plane, d_cands, d_count, cap, thr, sec, n_cols, p->n_z, p->bin0);                     \
+    } while (0)
     switch (n_stage) {
-    case 1: k_harmsum<1, 4, 2><<<FDAS_HS_GRID(4), block, 0, st>>>(FDAS_HS_ARGS); break;
-    case 2: k_harmsum<2, 4, 2><<<FDAS_HS_GRID(4), block, 0, st>>>(FDAS_HS_ARGS); break;
-    case 3: k_harmsum<3, 4, 2><<<FDAS_HS_GRID(4), block, 0, st>>>(FDAS_HS_ARGS); break;
-    case 4: k_harmsum<4, 2, 2><<<FDAS_HS_GRID(2), block, 0, st>>>(FDAS_HS_ARGS); break;
+    case 1: FDAS_HS_LAUNCH(1, 4, 2); break;
+    case 2: FDAS_HS_LAUNCH(2, 4, 2); break;
+    case 3: FDAS_HS_LAUNCH(3, 4, 2); break;
+    case 4: FDAS_HS_LAUNCH(4, 2, 2); break;
     default:
-        if (variant == 1) k_harmsum<5, 4, 2><<<FDAS_HS_GRID(4), block, 0, st>>>(FDAS_HS_ARGS);
-        else k_harmsum<5, 2, 4><<<FDAS_HS_GRID(2), block, 0, st>>>(FDAS_HS_ARGS);     // measured best on B200
+        if (variant == 1) FDAS_HS_LAUNCH(5, 4, 2);
+        else FDAS_HS_LAUNCH(5, 2, 4);                    // 64-column tiles, 4 CTAs/SM: best of the variants timed on B200
         break;
     }
-#undef FDAS_HS_GRID
-#undef FDAS_HS_ARGS
+#undef FDAS_HS_LAUNCH
     FDAS_LAUNCH_CHECK();
     return FDAS_OK;
 }
