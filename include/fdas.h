@@ -132,7 +132,8 @@ int fdas_correlate(fdas_plan* plan, const float* d_spectrum, int32_t n_batch,
                    uint32_t capacity, void* d_workspace, void* stream);
 
 /* Incoherent harmonic summing (BJ:configs[4]; "pulse harmonics") of ONE
- * integer-bin plane float[n_z][n_bins] (FDAS_E_INVALID on an interbinned plan), for
+ * integer-bin plane float[n_z][n_bins] (FDAS_E_INVALID on an interbinned plan, or if the plane has
+ * 2^31 cells or more), for
  * H in {1,2,4,..,max_harm}, max_harm in {1,2,4,8,16}:
  *   k = bin0 + col, zeta = zi - (n_z-1)/2,
  *   k_h = floor((k h + H/2)/H), zeta_h = sgn(zeta) floor((|zeta| h + H/2)/H),

@@ -24,51 +24,113 @@ __device__ __noinline__ void push_cand_hs(fdas_cand* list, uint32_t* count, uint
 }
 
 // CHECK = true: edge tiles (first tile: k_h may fall below bin0; last tile: columns beyond n_cols).
+//
+// A warp takes a run of CONSECUTIVE rows of the tile (one lane = HS_CPT cells, columns col0 + 32 j).  For
+// stream h/H the source column k_h does not depend on the row, and the source row zeta_h is non-decreasing
+// in zeta and repeats over ~H/h consecutive rows.  So each stream keeps one pointer per thread that is
+// advanced by one plane row when zeta_h moves, and a stream whose zeta_h did not move keeps last row's
+// values: (16 + 8.5 (R-1))/R loads per cell for a run of R rows instead of 16, and no per-row index
+// arithmetic.  Whether zeta_h moved is the same for the whole warp; lane s works it out for slot s
+// (h, H of that slot) and one ballot hands the 16-bit answer to everybody:
+//   t = |zeta| h + H/2, zeta_h = sgn(zeta) (t >> log2 H); against the previous row (|zeta| - 1 for
+//   zeta > 0, |zeta| + 1 for zeta <= 0) it moved iff (t mod H) < h, resp. (t mod H) + h >= H.
+// Stage st (H = 2^st) occupies slots [H/2, H): slot = H/2 + (h - 1)/2 for odd h; slot 0 is P itself.
 template <int NST, int HS_CPT, bool CHECK>
 __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fdas_cand* __restrict__ cands,
                                              uint32_t* __restrict__ count, uint32_t cap, const HarmThr& thr,
                                              int n_cols, int n_z, int bin0, int tile, int zi_lo, int zi_hi)
 {
     constexpr int HS_COLS = 32 * HS_CPT;
-    const int col0 = tile * HS_COLS + threadIdx.x;
+    constexpr int HMAX = 1 << (NST - 1);
+    const int lane = threadIdx.x;
+    const int col0 = tile * HS_COLS + lane;
     const int zc = (n_z - 1) / 2;
     const int k = bin0 + col0;
-    constexpr int HMAX = 1 << (NST - 1);
-    for (int zi = zi_lo + threadIdx.y; zi < zi_hi; zi += blockDim.y) {
-        const int zeta = zi - zc, az = abs(zeta), sg = zeta < 0 ? -1 : 1;
-        // issue every gather of the row's HS_CPT cells first (all independent), then sum in stage order
-        float v[HS_CPT][HMAX];
-        const float* prow = plane + (size_t)zi * n_cols + col0;
+    const int rpw = (zi_hi - zi_lo + (int)blockDim.y - 1) / (int)blockDim.y;
+    const int r_begin = zi_lo + (int)threadIdx.y * rpw, r_end = min(zi_hi, r_begin + rpw);
+    if (r_begin >= r_end) return;                                      // the whole warp
+
+    // this lane's slot for the ballot (lanes 0 and >= HMAX never report a move)
+    int my_h = 0, my_H = 1;
+    if (lane >= 1 && lane < HMAX) {
+        my_H = 2 << (31 - __clz(lane));
+        my_h = 2 * (lane - (my_H >> 1)) + 1;
+    }
+    // one plane index per stream (n_z n_cols < 2^31, checked by the launcher), set ONE ROW BEFORE the first
+    // source row: the first row moves every stream
+    int idx[HMAX];
+    unsigned long long okmask = 0;                                     // CHECK only: bit slot*HS_CPT + j = cell may be read
+    {
+        const int zeta0 = r_begin - zc, az0 = abs(zeta0), sg0 = zeta0 < 0 ? -1 : 1;
+        idx[0] = r_begin * n_cols + col0;
 #pragma unroll
-        for (int j = 0; j < HS_CPT; j++) v[j][0] = (!CHECK || col0 + 32 * j < n_cols) ? __ldcs(prow + 32 * j) : 0.0f;
+        for (int j = 0; j < HS_CPT; j++)
+            if (col0 + 32 * j < n_cols) okmask |= 1ull << j;
 #pragma unroll
         for (int st = 1; st < NST; st++) {
             const int H = 1 << st;
 #pragma unroll
             for (int h = 1; h < H; h += 2) {
+                const int slot = (H >> 1) + (h >> 1);
                 const int kh = (k * h + (H >> 1)) >> st;              // k*h < 2^29 for n_samples <= 2^25
-                const int zh = sg * ((az * h + (H >> 1)) >> st);
-                const float* src = plane + (size_t)(zc + zh) * n_cols + (kh - bin0);
-                const int dk = (32 * h) >> st;                         // exact: 32 h / H
+                const int zh0 = sg0 * ((az0 * h + (H >> 1)) >> st);
+                idx[slot] = (zc + zh0 - 1) * n_cols + (kh - bin0);
+                if (CHECK) {
 #pragma unroll
-                for (int j = 0; j < HS_CPT; j++) {
-                    float x = 0.0f;
-                    if (!CHECK || (kh + dk * j >= bin0 && col0 + 32 * j < n_cols)) x = __ldg(src + dk * j);
-                    v[j][(H >> 1) + (h >> 1)] = x;                     // stage st occupies slots [H/2, H)
+                    for (int j = 0; j < HS_CPT; j++)
+                        if (kh + ((32 * h) >> st) * j >= bin0 && col0 + 32 * j < n_cols) okmask |= 1ull << (slot * HS_CPT + j);
+                }
+            }
+        }
+    }
+    float v[HS_CPT][HMAX];
+    for (int zi = r_begin; zi < r_end; zi++) {
+        const int zeta = zi - zc;
+        const int t = abs(zeta) * my_h + (my_H >> 1), fr = t & (my_H - 1);
+        unsigned moved = __ballot_sync(0xffffffffu, zeta > 0 ? fr < my_h : fr + my_h >= my_H);
+        if (zi == r_begin) moved = 0xffffffffu;
+        // issue every gather of the row first (all independent), then sum in stage order
+        {
+            const float* src = plane + idx[0];
+#pragma unroll
+            for (int j = 0; j < HS_CPT; j++) v[j][0] = (!CHECK || (okmask >> j & 1)) ? __ldcs(src + 32 * j) : 0.0f;
+            idx[0] += n_cols;
+        }
+#pragma unroll
+        for (int st = 1; st < NST; st++) {
+            const int H = 1 << st;
+#pragma unroll
+            for (int h = 1; h < H; h += 2) {
+                const int slot = (H >> 1) + (h >> 1);
+                if (moved & (1u << slot)) {                            // warp-uniform
+                    idx[slot] += n_cols;
+                    const float* src = plane + idx[slot];
+                    const int dk = (32 * h) >> st;                     // exact: 32 h / H
+#pragma unroll
+                    for (int j = 0; j < HS_CPT; j++)
+                        v[j][slot] = (!CHECK || (okmask >> (slot * HS_CPT + j) & 1)) ? __ldg(src + dk * j) : 0.0f;
                 }
             }
         }
 #pragma unroll
         for (int j = 0; j < HS_CPT; j++) {
+            // the stage sums, and ONE branch for the (rare) cell that passes any threshold
+            float sum[NST];
             float acc = v[j][0];
-            const bool ok = !CHECK || col0 + 32 * j < n_cols;
-            if (acc > thr.t[0] && ok) push_cand_hs(cands, count, cap, col0 + 32 * j, zi, 1, acc);
+            sum[0] = acc;
+            bool any = acc > thr.t[0];
 #pragma unroll
             for (int st = 1; st < NST; st++) {
                 const int H = 1 << st;
 #pragma unroll
                 for (int i = H >> 1; i < H; i++) acc += v[j][i];
-                if (acc > thr.t[st] && ok) push_cand_hs(cands, count, cap, col0 + 32 * j, zi, H, acc);
+                sum[st] = acc;
+                any = any || acc > thr.t[st];
+            }
+            if (any && (!CHECK || (okmask >> j & 1))) {
+#pragma unroll
+                for (int st = 0; st < NST; st++)
+                    if (sum[st] > thr.t[st]) push_cand_hs(cands, count, cap, col0 + 32 * j, zi, 1 << st, sum[st]);
             }
         }
     }
@@ -82,15 +144,15 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
 // are swept one after the other, columns ascending inside each.  Boundary ray j = 0..S is named by where it
 // leaves the rectangle [0, K] x [-n_z/2, n_z/2], u_j = -2 + 4 j/S:  |u| <= 1: through the far edge k = K at
 // row (n_z/2) u;  1 < |u| <= 2: through the top/bottom edge at column K (2 - |u|)  (|u| = 2: vertical).
-// Sector s holds, in the column tile whose last bin is kc, the rows ceil(zb_s(kc)) <= zeta < ceil(zb_{s+1}(kc))
+// Sector s holds, in the CTA column range whose last bin is kc, the rows ceil(zb_s(kc)) <= zeta < ceil(zb_{s+1}(kc))
 // -- a partition of the rows of every tile.  A sector is thin, so the span of plane that streams through L2
 // between two uses of a source cell fits (the same model: 1.54 GB at S = 16, 1.43-1.51 GB at S = 32 for a
 // 90-60 MB cache: the plane is read from DRAM about once).  S = 1 is the plain order; results do not depend on S.
 constexpr int HS_MAX_SECTORS = 64;
-constexpr int HS_TILES_PER_CTA = 8;      // consecutive column tiles of its sector per CTA (a sector is only a few rows thin)
+constexpr int HS_COLS_PER_CTA = 512;     // consecutive columns of its sector per CTA (a sector is only a few rows thin)
 struct HarmSectors {
-    int n_sec;
-    int first_cta[HS_MAX_SECTORS + 1];       // sector s owns CTAs [first_cta[s], first_cta[s+1]), HS_TILES_PER_CTA column tiles each
+    int n_sec, tiles_per_cta;
+    int first_cta[HS_MAX_SECTORS + 1];       // sector s owns CTAs [first_cta[s], first_cta[s+1]), tiles_per_cta column tiles each
 };
 
 __host__ __device__ inline double sector_boundary(int j, int S, double kc, double K, double zhalf)
@@ -111,18 +173,19 @@ k_harmsum(const float* __restrict__ plane, fdas_cand* __restrict__ cands, uint32
     int s = 0;
     while (s + 1 < sec.n_sec && (int)blockIdx.x >= sec.first_cta[s + 1]) s++;      // CTA-uniform, <= 63 steps
     const int n_tiles = (n_cols + HS_COLS - 1) / HS_COLS;
-    const int tile0 = (blockIdx.x - sec.first_cta[s]) * HS_TILES_PER_CTA;
-    const int zc = (n_z - 1) / 2;
-    const double K = (double)(bin0 + n_cols - 1), zhalf = 0.5 * (double)n_z;
+    const int tile0 = (blockIdx.x - sec.first_cta[s]) * sec.tiles_per_cta;
+    const int tile1 = min(n_tiles, tile0 + sec.tiles_per_cta);
+    int zi_lo = 0, zi_hi = n_z;
+    if (sec.n_sec > 1) {                     // rows of this sector, taken at the last bin of the CTA's column range
+        const int zc = (n_z - 1) / 2;
+        const double K = (double)(bin0 + n_cols - 1), zhalf = 0.5 * (double)n_z;
+        const double kc = (double)bin0 + (double)min(n_cols, tile1 * HS_COLS) - 1.0;
+        zi_lo = max(0, min(n_z, (int)ceil(sector_boundary(s, sec.n_sec, kc, K, zhalf)) + zc));
+        zi_hi = max(0, min(n_z, (int)ceil(sector_boundary(s + 1, sec.n_sec, kc, K, zhalf)) + zc));
+        if (zi_lo >= zi_hi) return;                                                // CTA-uniform
+    }
 #pragma unroll 1
-    for (int tile = tile0; tile < min(n_tiles, tile0 + HS_TILES_PER_CTA); tile++) {
-        int zi_lo = 0, zi_hi = n_z;
-        if (sec.n_sec > 1) {
-            const double kc = (double)bin0 + (double)min(n_cols, (tile + 1) * HS_COLS) - 1.0;
-            zi_lo = max(0, min(n_z, (int)ceil(sector_boundary(s, sec.n_sec, kc, K, zhalf)) + zc));
-            zi_hi = max(0, min(n_z, (int)ceil(sector_boundary(s + 1, sec.n_sec, kc, K, zhalf)) + zc));
-            if (zi_lo >= zi_hi) continue;                                          // CTA-uniform
-        }
+    for (int tile = tile0; tile < tile1; tile++) {
         const bool edge = tile == 0 || tile * HS_COLS + HS_COLS > n_cols;          // CTA-uniform
         if (edge) harmsum_tile<NST, HS_CPT, true>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi);
         else harmsum_tile<NST, HS_CPT, false>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi);
@@ -135,6 +198,7 @@ static HarmSectors make_sectors(int n_sec, int n_cols, int bin0, int cols_per_ti
 {
     HarmSectors hs;
     hs.n_sec = n_sec;
+    hs.tiles_per_cta = HS_COLS_PER_CTA / cols_per_tile;
     const int n_tiles = (n_cols + cols_per_tile - 1) / cols_per_tile;
     const double K = (double)(bin0 + n_cols - 1);
     hs.first_cta[0] = 0;
@@ -146,11 +210,11 @@ static HarmSectors make_sectors(int n_sec, int n_cols, int bin0, int cols_per_ti
             bool same_side = (-2.0 + 4.0 * s / n_sec) * (-2.0 + 4.0 * (s + 1) / n_sec) > 0.0;
             if (same_side && umin > 1.0) {
                 double c_outer = K * (2.0 - umin);
-                long long t = (long long)(c_outer / cols_per_tile) + 2;
+                long long t = ((long long)(c_outer / HS_COLS_PER_CTA) + 2) * hs.tiles_per_cta;
                 if (t < nt) nt = (int)t;
             }
         }
-        hs.first_cta[s + 1] = hs.first_cta[s] + (nt + HS_TILES_PER_CTA - 1) / HS_TILES_PER_CTA;
+        hs.first_cta[s + 1] = hs.first_cta[s] + (nt + hs.tiles_per_cta - 1) / hs.tiles_per_cta;
     }
     return hs;
 }
@@ -182,6 +246,7 @@ k_candidates(const float* __restrict__ plane, fdas_cand* __restrict__ cands, uin
 int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const float* h_thr,
                         fdas_cand* d_cands, uint32_t* d_count, uint32_t cap, cudaStream_t st)
 {
+    if ((long long)p->n_z * p->n_cols > 0x7fffffffLL) return FDAS_E_INVALID;          // 32-bit plane indices in the kernel
     int n_stage = 0;
     for (int H = 1; H <= max_harm; H <<= 1) n_stage++;
     HarmThr thr;
@@ -195,7 +260,7 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     static const int env_rows = getenv("FDAS_HS_ROWS") ? atoi(getenv("FDAS_HS_ROWS")) : 0;
     int n_sec = env_sectors < 1 ? 1 : env_sectors;
     if (n_sec > HS_MAX_SECTORS) n_sec = HS_MAX_SECTORS;
-    int rows = env_rows > 0 ? env_rows : (n_sec == 1 ? HS_ROWS_PER_PASS : 4);      // warps per CTA, one row each per pass
+    int rows = env_rows > 0 ? env_rows : (n_sec == 1 ? HS_ROWS_PER_PASS : 2);      // warps per CTA; each takes a run of consecutive rows
     if (rows > HS_ROWS_PER_PASS) rows = HS_ROWS_PER_PASS;
     dim3 block(32, rows);
     HarmSectors sec;
@@ -212,7 +277,7 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     case 4: FDAS_HS_LAUNCH(4, 2, 2); break;
     default:
         if (variant == 1) FDAS_HS_LAUNCH(5, 4, 2);
-        else FDAS_HS_LAUNCH(5, 2, 4);                    // 64-column tiles, 4 CTAs/SM: best of the variants timed on B200
+        else FDAS_HS_LAUNCH(5, 2, 2);                    // 64-column tiles, 118 registers, no spills (cuobjdump: ~90 instructions per cell and row)
         break;
     }
 #undef FDAS_HS_LAUNCH

@@ -67,6 +67,13 @@ void emu_syncwarp();
 void* emu_dyn_smem();
 void emu_check_ptr(const void* p, size_t n, const char* what);
 void emu_launch(dim3 grid, dim3 block, size_t smem, const char* name, const std::function<void()>& body);
+unsigned emu_ballot(int pred);
+static inline unsigned __ballot_sync(unsigned mask, int pred)
+{
+    if (mask != 0xffffffffu) { fprintf(stderr, "EMU: __ballot_sync with a partial mask is not modelled\n"); abort(); }
+    return emu_ballot(pred);
+}
+static inline int __clz(int x) { return x ? __builtin_clz((unsigned)x) : 32; }
 #define __syncthreads() emu_syncthreads()
 #define __syncwarp() emu_syncwarp()
 

@@ -123,9 +123,10 @@ static void ctx_make(Ctx* c, char* stack, size_t size, void (*fn)(), Ctx* link)
     makecontext(&c->uc, fn, 0);
 }
 #endif
-struct Fiber { Ctx ctx; char* stack; int state; uint3 tid; };
+struct Fiber { Ctx ctx; char* stack; int state; uint3 tid; unsigned n_ballot; };
 struct Worker {
     std::vector<Fiber> fibers;
+    std::vector<unsigned> ballot;            // [warp][2]: alternating accumulators of __ballot_sync
     Ctx sched;
     int cur;
     const std::function<void()>* body;
@@ -153,6 +154,22 @@ void emu_syncthreads() { yield_with(ST_BLOCK_BAR); }
 void emu_syncwarp() { yield_with(ST_WARP_BAR); }
 void* emu_dyn_smem() { return t_w->dyn_smem; }
 
+// __ballot_sync over the full warp: OR this lane's bit into the warp's accumulator, meet at a warp barrier,
+// read; the other accumulator is cleared for the next ballot between the two barriers (nobody uses it then).
+unsigned emu_ballot(int pred)
+{
+    Worker* w = t_w;
+    const int i = w->cur, warp = i / 32, lane = i % 32;
+    const unsigned cur = w->fibers[i].n_ballot++ & 1u;
+    if (pred) w->ballot[2 * warp + cur] |= 1u << lane;
+    yield_with(ST_WARP_BAR);
+    w = t_w;
+    const unsigned r = w->ballot[2 * warp + cur];
+    w->ballot[2 * warp + (cur ^ 1u)] = 0;
+    yield_with(ST_WARP_BAR);
+    return r;
+}
+
 static void run_block(Worker* w, dim3 block, bool rev)
 {
     const int nt = block.x * block.y * block.z;
@@ -165,8 +182,10 @@ static void run_block(Worker* w, dim3 block, bool rev)
         Fiber& f = w->fibers[i];
         ctx_make(&f.ctx, f.stack, STACK, tramp, &w->sched);
         f.state = ST_RUN;
+        f.n_ballot = 0;
         f.tid = uint3{(unsigned)i % block.x, ((unsigned)i / block.x) % block.y, (unsigned)i / (block.x * block.y)};
     }
+    w->ballot.assign(2 * ((nt + 31) / 32), 0u);
     int done = 0;
     while (done < nt) {
         bool progress = false;
