@@ -292,6 +292,31 @@ def test_config3_fused_batch(fdas):
         assert_cand_parity(fdas.cands_to_numpy(cands[0], cands[1], d), c_ref, lambda h: 15.0)
 
 
+def test_maximum_series_length(fdas):
+    """The largest series the plan accepts (2^25 samples; 2^24 columns per row): index arithmetic at its
+    limits (k h, plane indices, twiddle phases), 3 templates to keep the oracle's share small."""
+    N = 1 << 25
+    x = synth.make_series(N, 77, [synth.Signal(0.02, 9.0e6 + 0.25, 1.5, 0.3), synth.Signal(0.02, 1.6e7 - 3.5, -2.0, 1.0)])
+    plan = fdas.Plan(N, 2.0, 2.0, 256, 2048)
+    d_P, c_gpu = run_gpu_plane(fdas, plan, x, thr=30.0)
+    S, _ = oracle.spectrum(x)
+    T = oracle.templates(2.0, 2.0, 256)
+    P_ref = oracle.correlate_fft(S, T, 2048)
+    pmax = float(P_ref.max())
+    for c0 in (0, (1 << 24) - 2048, 9_000_000 - 1024):
+        Pd = oracle.correlate_direct(S, T, c0=c0, nc=2048)
+        assert np.max(np.abs(Pd - P_ref[:, c0:c0 + 2048])) <= 1e-10 * pmax
+    for zi in range(3):
+        assert_power_parity(d_P[zi].cpu().numpy(), P_ref[zi], pmax)
+    assert_cand_parity(c_gpu, oracle.candidates(P_ref, 30.0), lambda h: 30.0)
+    thr = oracle.thresholds(16)
+    cands = plan.empty_cands(1 << 20)
+    plan.harmsum(d_P, 16, thr, cands, 1 << 20)
+    thr32 = thr.astype(np.float32)
+    assert_cand_parity(fdas.cands_to_numpy(*cands), oracle.harmsum(P_ref, 16, thr, bin0=1),
+                       lambda h: float(thr32[int(h).bit_length() - 1]))
+
+
 def test_search_host_matches_device_calls(fdas):
     cfg = synth.config(0)
     x = cfg.series()
