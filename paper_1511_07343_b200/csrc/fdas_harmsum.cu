@@ -276,7 +276,7 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     case 3: FDAS_HS_LAUNCH(3, 4, 2); break;
     case 4: FDAS_HS_LAUNCH(4, 2, 2); break;
     default:
-        if (variant == 1) FDAS_HS_LAUNCH(5, 4, 2);
+        if (variant == 1) FDAS_HS_LAUNCH(5, 4, 1);        // 128-column tiles, ~190 registers, ~67 instructions per cell: to be timed against the default
         else FDAS_HS_LAUNCH(5, 2, 2);                    // 64-column tiles, 118 registers, no spills (cuobjdump: ~90 instructions per cell and row)
         break;
     }
