@@ -71,6 +71,12 @@ class Signal:
     phi: float = 0.0
 
 
+def pulse_train(amp: float, r0: float, z0: float, n_harm: int, decay: float = 1.0, phi: float = 0.0):
+    """The first `n_harm` harmonics of an accelerated pulsar: harmonic h sits at (h r0, h z0) with amplitude
+    amp * decay^(h-1) ("pulse harmonics"; z scales with the frequency)."""
+    return [Signal(amp * decay ** (h - 1), h * r0, h * z0, phi * h) for h in range(1, n_harm + 1)]
+
+
 def make_series(n_samples: int, seed: int, signals=(), noise: bool = True,
                 chunk: int = 1 << 21) -> np.ndarray:
     """float32[n_samples] = N(0,1) noise (stream `seed`) + the given signals."""

@@ -292,6 +292,26 @@ def test_config3_fused_batch(fdas):
         assert_cand_parity(fdas.cands_to_numpy(cands[0], cands[1], d), c_ref, lambda h: 15.0)
 
 
+def test_pulse_train_is_found_by_the_harmonic_sum(fdas):
+    """Multi-harmonic workload for row a7: eight harmonics of a fundamental at bin
+    250, z0 = 1, in N(0,1) noise; candidates as the oracle's, and the most significant one is the
+    8-harmonic sum labelled by the top harmonic (8 r0, 8 z0)."""
+    N, r0, z0, nh = 1 << 14, 250, 1, 8
+    x = synth.make_series(N, 4711, synth.pulse_train(0.055, r0, z0, nh, phi=0.4))
+    plan = fdas.Plan(N, 8.0, 1.0, 64, 2048)
+    d_P, _ = run_gpu_plane(fdas, plan, x)
+    thr = oracle.thresholds(16, 1e-5)
+    cands = plan.empty_cands(1 << 14)
+    plan.harmsum(d_P, 16, thr, cands, 1 << 14)
+    c = fdas.cands_to_numpy(*cands)
+    S, _ = oracle.spectrum(x)
+    c_ref = oracle.harmsum(oracle.correlate_direct(S, oracle.templates(8.0, 1.0, 64)), 16, thr, bin0=1)
+    thr32 = thr.astype(np.float32)
+    assert_cand_parity(c, c_ref, lambda h: float(thr32[int(h).bit_length() - 1]))
+    best = min(c, key=lambda r: oracle.gamma_q(int(r["nharm"]), float(r["power"])))
+    assert (int(best["nharm"]), int(best["col"]), int(best["zi"])) == (8, r0 * nh - 1, 8 + z0 * nh)
+
+
 def test_maximum_series_length(fdas):
     """The largest series the plan accepts (2^25 samples; 2^24 columns per row): index arithmetic at its
     limits (k h, plane indices, twiddle phases), 3 templates to keep the oracle's share small."""
