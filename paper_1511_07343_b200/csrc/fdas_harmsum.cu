@@ -144,15 +144,19 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
 // are swept one after the other, columns ascending inside each.  Boundary ray j = 0..S is named by where it
 // leaves the rectangle [0, K] x [-n_z/2, n_z/2], u_j = -2 + 4 j/S:  |u| <= 1: through the far edge k = K at
 // row (n_z/2) u;  1 < |u| <= 2: through the top/bottom edge at column K (2 - |u|)  (|u| = 2: vertical).
-// Sector s holds, in the CTA column range whose last bin is kc, the rows ceil(zb_s(kc)) <= zeta < ceil(zb_{s+1}(kc))
+// Sector s holds, in the column tile whose last bin is kc, the rows ceil(zb_s(kc)) <= zeta < ceil(zb_{s+1}(kc))
 // -- a partition of the rows of every tile.  A sector is thin, so the span of plane that streams through L2
 // between two uses of a source cell fits (the same model: 1.54 GB at S = 16, 1.43-1.51 GB at S = 32 for a
 // 90-60 MB cache: the plane is read from DRAM about once).  S = 1 is the plain order; results do not depend on S.
+// The kernel is PERSISTENT: the grid holds as many CTAs as are resident at once and CTA c takes the work
+// items c, c + gridDim.x, ... (item = one 32 HS_CPT-column tile of one sector, sector-major, columns
+// ascending).  So the CTAs running at any moment work on ~gridDim.x consecutive tiles (~76 k columns of one
+// sector) and advance together, which is what the reuse argument needs; one CTA per run of tiles would spread
+// the resident CTAs over a quarter of the plane.
 constexpr int HS_MAX_SECTORS = 64;
-constexpr int HS_COLS_PER_CTA = 512;     // consecutive columns of its sector per CTA (a sector is only a few rows thin)
 struct HarmSectors {
-    int n_sec, tiles_per_cta;
-    int first_cta[HS_MAX_SECTORS + 1];       // sector s owns CTAs [first_cta[s], first_cta[s+1]), tiles_per_cta column tiles each
+    int n_sec;
+    int first_item[HS_MAX_SECTORS + 1];      // sector s owns items [first_item[s], first_item[s+1]): its column tiles 0, 1, ...
 };
 
 __host__ __device__ inline double sector_boundary(int j, int S, double kc, double K, double zhalf)
@@ -170,53 +174,62 @@ k_harmsum(const float* __restrict__ plane, fdas_cand* __restrict__ cands, uint32
           uint32_t cap, HarmThr thr, HarmSectors sec, int n_cols, int n_z, int bin0)
 {
     constexpr int HS_COLS = 32 * HS_CPT;
+    const int zc = (n_z - 1) / 2;
+    const double K = (double)(bin0 + n_cols - 1), zhalf = 0.5 * (double)n_z;
+    const int n_items = sec.first_item[sec.n_sec];
     int s = 0;
-    while (s + 1 < sec.n_sec && (int)blockIdx.x >= sec.first_cta[s + 1]) s++;      // CTA-uniform, <= 63 steps
-    const int n_tiles = (n_cols + HS_COLS - 1) / HS_COLS;
-    const int tile0 = (blockIdx.x - sec.first_cta[s]) * sec.tiles_per_cta;
-    const int tile1 = min(n_tiles, tile0 + sec.tiles_per_cta);
-    int zi_lo = 0, zi_hi = n_z;
-    if (sec.n_sec > 1) {                     // rows of this sector, taken at the last bin of the CTA's column range
-        const int zc = (n_z - 1) / 2;
-        const double K = (double)(bin0 + n_cols - 1), zhalf = 0.5 * (double)n_z;
-        const double kc = (double)bin0 + (double)min(n_cols, tile1 * HS_COLS) - 1.0;
-        zi_lo = max(0, min(n_z, (int)ceil(sector_boundary(s, sec.n_sec, kc, K, zhalf)) + zc));
-        zi_hi = max(0, min(n_z, (int)ceil(sector_boundary(s + 1, sec.n_sec, kc, K, zhalf)) + zc));
-        if (zi_lo >= zi_hi) return;                                                // CTA-uniform
-    }
 #pragma unroll 1
-    for (int tile = tile0; tile < tile1; tile++) {
-        const bool edge = tile == 0 || tile * HS_COLS + HS_COLS > n_cols;          // CTA-uniform
+    for (int item = blockIdx.x; item < n_items; item += gridDim.x) {                // everything here is CTA-uniform
+        while (item >= sec.first_item[s + 1]) s++;
+        const int tile = item - sec.first_item[s];
+        int zi_lo = 0, zi_hi = n_z;
+        if (sec.n_sec > 1) {                 // rows of this sector, taken at the last bin of the tile
+            const double kc = (double)bin0 + (double)min(n_cols, (tile + 1) * HS_COLS) - 1.0;
+            zi_lo = max(0, min(n_z, (int)ceil(sector_boundary(s, sec.n_sec, kc, K, zhalf)) + zc));
+            zi_hi = max(0, min(n_z, (int)ceil(sector_boundary(s + 1, sec.n_sec, kc, K, zhalf)) + zc));
+            if (zi_lo >= zi_hi) continue;
+        }
+        const bool edge = tile == 0 || tile * HS_COLS + HS_COLS > n_cols;
         if (edge) harmsum_tile<NST, HS_CPT, true>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi);
         else harmsum_tile<NST, HS_CPT, false>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi);
     }
 }
 
-// Sector -> CTA ranges.  A sector whose two boundary rays both leave through the top/bottom edge is empty
-// beyond the column where the shallower one leaves; only the tiles before that are launched.
+// Sector -> item ranges.  A sector whose two boundary rays both leave through the top/bottom edge is empty
+// beyond the column where the shallower one leaves; only the tiles before that become items.
 static HarmSectors make_sectors(int n_sec, int n_cols, int bin0, int cols_per_tile)
 {
     HarmSectors hs;
     hs.n_sec = n_sec;
-    hs.tiles_per_cta = HS_COLS_PER_CTA / cols_per_tile;
     const int n_tiles = (n_cols + cols_per_tile - 1) / cols_per_tile;
     const double K = (double)(bin0 + n_cols - 1);
-    hs.first_cta[0] = 0;
+    hs.first_item[0] = 0;
     for (int s = 0; s < n_sec; s++) {
         int nt = n_tiles;
         if (n_sec > 1) {
-            double u0 = fabs(-2.0 + 4.0 * s / n_sec), u1 = fabs(-2.0 + 4.0 * (s + 1) / n_sec);
-            double umin = u0 < u1 ? u0 : u1;
-            bool same_side = (-2.0 + 4.0 * s / n_sec) * (-2.0 + 4.0 * (s + 1) / n_sec) > 0.0;
-            if (same_side && umin > 1.0) {
-                double c_outer = K * (2.0 - umin);
-                long long t = ((long long)(c_outer / HS_COLS_PER_CTA) + 2) * hs.tiles_per_cta;
+            const double ua = -2.0 + 4.0 * s / n_sec, ub = -2.0 + 4.0 * (s + 1) / n_sec;
+            const double umin = fabs(ua) < fabs(ub) ? fabs(ua) : fabs(ub);
+            if (ua * ub > 0.0 && umin > 1.0) {
+                const long long t = (long long)(K * (2.0 - umin) / cols_per_tile) + 2;
                 if (t < nt) nt = (int)t;
             }
         }
-        hs.first_cta[s + 1] = hs.first_cta[s] + (nt + hs.tiles_per_cta - 1) / hs.tiles_per_cta;
+        hs.first_item[s + 1] = hs.first_item[s] + nt;
     }
     return hs;
+}
+
+// CTAs resident at once for kernel `k` with `threads` per CTA (the persistent grid).
+template <class K>
+static int resident_ctas(K k, int threads)
+{
+    int dev = 0, sms = 0, per_sm = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess ||
+        cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, threads, 0) != cudaSuccess || sms < 1 || per_sm < 1) {
+        cudaGetLastError();
+        return 148 * 4;
+    }
+    return sms * per_sm;
 }
 
 // Threshold + compaction over one plane (row a8). grid-stride over float4 groups of a row.
@@ -267,7 +280,9 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
 #define FDAS_HS_LAUNCH(NST, CPT, MINB)                                                              \
     do {                                                                                            \
         sec = make_sectors(n_sec, n_cols, p->bin0, 32 * CPT);                                       \
-        k_harmsum<NST, CPT, MINB><<<dim3(sec.first_cta[n_sec]), block, 0, st>>>(                    \
+        int n_cta = resident_ctas(k_harmsum<NST, CPT, MINB>, 32 * rows);                            \
+        if (n_cta > sec.first_item[n_sec]) n_cta = sec.first_item[n_sec];                           \
+        k_harmsum<NST, CPT, MINB><<<dim3(n_cta), block, 0, st>>>(                                   \
             d_plane, d_cands, d_count, cap, thr, sec, n_cols, p->n_z, p->bin0);                     \
     } while (0)
     switch (n_stage) {
