@@ -273,7 +273,7 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     static const int env_rows = getenv("FDAS_HS_ROWS") ? atoi(getenv("FDAS_HS_ROWS")) : 0;
     int n_sec = env_sectors < 1 ? 1 : env_sectors;
     if (n_sec > HS_MAX_SECTORS) n_sec = HS_MAX_SECTORS;
-    int rows = env_rows > 0 ? env_rows : (n_sec == 1 ? HS_ROWS_PER_PASS : 2);      // warps per CTA; each takes a run of consecutive rows
+    int rows = env_rows > 0 ? env_rows : (n_sec == 1 ? HS_ROWS_PER_PASS : 1);      // warps per CTA; each takes a run of consecutive rows (all rows of a sector tile: longest runs)
     if (rows > HS_ROWS_PER_PASS) rows = HS_ROWS_PER_PASS;
     dim3 block(32, rows);
     HarmSectors sec;
