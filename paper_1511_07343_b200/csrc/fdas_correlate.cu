@@ -227,18 +227,25 @@ __device__ __forceinline__ void v2_pass3(const float2* buf, const float2* tw_a, 
     }
     dit_tw<8>(u0, tw_a);
     dit_tw<8>(u1, tw_b);
+    float pa[8], pb[8];
+    float mx = 0.0f;                                   // largest kept power of this thread (fused threshold: one test)
 #pragma unroll
     for (int t3 = 0; t3 < 8; t3++) {
         if (FULL ? (t3 >= NKEEP) : (t3 >= nv)) continue;
-        const float pa = fmaf(u0[t3].x, u0[t3].x, u0[t3].y * u0[t3].y);
-        const float pb = fmaf(u1[t3].x, u1[t3].x, u1[t3].y * u1[t3].y);
+        pa[t3] = fmaf(u0[t3].x, u0[t3].x, u0[t3].y * u0[t3].y);
+        pb[t3] = fmaf(u1[t3].x, u1[t3].x, u1[t3].y * u1[t3].y);
         if (HAS_PLANE) {
-            if (NSET == 1) *reinterpret_cast<float2*>(prow + 256 * t3) = make_float2(pa, pb);
-            else { prow[(256 * t3) * NSET] = pa; prow[(256 * t3 + 1) * NSET] = pb; }
+            if (NSET == 1) *reinterpret_cast<float2*>(prow + 256 * t3) = make_float2(pa[t3], pb[t3]);
+            else { prow[(256 * t3) * NSET] = pa[t3]; prow[(256 * t3 + 1) * NSET] = pb[t3]; }
         }
-        if (HAS_CANDS) {
-            if (pa > thr) push_cand_slow(cands, counts, cap, col0 + 256 * t3 * NSET, zi, pa);
-            if (pb > thr) push_cand_slow(cands, counts, cap, col0 + (256 * t3 + 1) * NSET, zi, pb);
+        if (HAS_CANDS) mx = fmaxf(mx, fmaxf(pa[t3], pb[t3]));
+    }
+    if (HAS_CANDS && mx > thr) {                       // rare
+#pragma unroll
+        for (int t3 = 0; t3 < 8; t3++) {
+            if (FULL ? (t3 >= NKEEP) : (t3 >= nv)) continue;
+            if (pa[t3] > thr) push_cand_slow(cands, counts, cap, col0 + 256 * t3 * NSET, zi, pa[t3]);
+            if (pb[t3] > thr) push_cand_slow(cands, counts, cap, col0 + (256 * t3 + 1) * NSET, zi, pb[t3]);
         }
     }
 }
