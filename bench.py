@@ -228,7 +228,9 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     ms = e0.elapsed_time(e1)
-    stage = np.array([[m[j].elapsed_time(m[j + 1]) for j in range(3)] for m in marks]).mean(axis=0)
+    stage_all = np.array([[m[j].elapsed_time(m[j + 1]) for j in range(3)] for m in marks])
+    stage = stage_all.mean(axis=0)
+    fp32_measured, _ = fdas.fdas_measure_fp32_tflops()       # FFMA-chain microbenchmark (untimed region)
     n_found = int(cands[1][0])
 
     # BASELINE.json configs[3] (streaming batch, plane not stored, threshold fused into the segment kernel):
@@ -308,6 +310,7 @@ def run_ours(args):
                      "achieved": (4 * cfg.n_samples + 8 * info.n_bins) / (spec_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s"},
         "correlate": {"kernels": "k_correlate_2048_v2", "bound": "alu", "ms": corr_ms, "algorithmic_flops": flops,
                       "achieved": corr_tf, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
+                      "peak_measured_ffma": fp32_measured, "frac_of_measured_ffma": corr_tf / fp32_measured,
                       "hbm_side": {"bytes": plane_bytes + 8 * info.n_bins,
                                    "achieved_gbs": (plane_bytes + 8 * info.n_bins) / (corr_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak}},
         "harmsum": {"kernels": "k_harmsum<5,...>", "bound": "hbm", "ms": hs_ms, "algorithmic_bytes": plane_bytes,
@@ -341,6 +344,9 @@ def run_ours(args):
                    "parallelism": "DM trials sharded across ranks, no collective"},
         "plane_outputs_per_s": world * info.n_templates * info.n_bins / (corr_ms * 1e-3),
         "stage_ms": {"spectrum": spec_ms, "correlate": corr_ms, "harmsum": hs_ms},
+        "stage_ms_median": dict(zip(("spectrum", "correlate", "harmsum"), (float(v) for v in np.median(stage_all, axis=0)))),
+        "stage_ms_min": dict(zip(("spectrum", "correlate", "harmsum"), (float(v) for v in stage_all.min(axis=0)))),
+        "fp32_peak": {"nominal_tflops": FP32_PEAK_TFLOPS, "measured_ffma_tflops": fp32_measured},
         "fft_correlation_roofline": {"ms_at_roofline": t_roof_ms, "ms_measured": spec_ms + corr_ms,
                                      "frac": t_roof_ms / (spec_ms + corr_ms),
                                      "dm_trials_per_s_without_harmsum": world * 1e3 / (spec_ms + corr_ms)},

@@ -166,6 +166,13 @@ int fdas_search_host(fdas_plan* plan, const float* h_series, int32_t n_batch, in
  * (BJ:configs[4]). Host computation in fp64; returns NaN for H < 1 or pfa outside (0,1). */
 double fdas_threshold(int32_t n_harm, double pfa);
 
+/* Measurement aid: the FP32 fused-multiply-add rate of the current device in
+ * TFLOP/s, from a kernel of independent FFMA chains (a <- a*x + y) on every SM, best of 4 timed
+ * launches with CUDA events on `stream`; *out_ms (may be NULL) receives that launch's duration.
+ * bench.py reports the fused correlate kernel against this measured peak as well as the nominal one.
+ * Synchronises `stream`; allocates and frees 4 bytes of device memory.  Not part of the search path. */
+int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, void* stream);
+
 int fdas_plan_destroy(fdas_plan* plan);
 
 /* Static text for an FDAS_E_* code; for FDAS_E_CUDA the text of the last CUDA error seen. */

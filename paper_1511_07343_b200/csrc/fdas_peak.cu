@@ -1,0 +1,62 @@
+// fdas_peak.cu -- FP32 FMA-rate microbenchmark ("the builder must add an
+// FFMA-chain microbenchmark, record the measured FP32 peak").  It gives bench.py a MEASURED
+// denominator for the ALU-bound fused correlate kernel beside the nominal 148 x 128 x 2 x clock.
+// Measurement aid only: nothing on the search path calls it.
+#include "fdas_common.cuh"
+
+constexpr int PEAK_ACC = 16;           // independent accumulators per thread (FMA latency 4 x 4 warps per scheduler)
+
+// Every thread runs `iters` rounds of PEAK_ACC fused multiply-adds a <- a*x + y with loop-invariant x, y
+// (the operand pattern of the FFT butterflies: two invariant twiddle registers, one running value).
+__global__ void __launch_bounds__(256)
+k_ffma_peak(float* __restrict__ sink, float x, float y, int iters)
+{
+    float a[PEAK_ACC];
+#pragma unroll
+    for (int i = 0; i < PEAK_ACC; i++) a[i] = (float)(threadIdx.x + i) * 1.0e-3f;
+#pragma unroll 1
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int r = 0; r < 4; r++) {
+#pragma unroll
+            for (int i = 0; i < PEAK_ACC; i++) a[i] = fmaf(a[i], x, y);
+        }
+    }
+    float s = 0.0f;
+#pragma unroll
+    for (int i = 0; i < PEAK_ACC; i++) s += a[i];
+    if (s == 123.456f) sink[0] = s;    // never true for the x, y used; keeps the chain alive
+}
+
+extern "C" int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, void* stream)
+{
+    if (!out_tflops) return FDAS_E_INVALID;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    FDAS_CUDA(cudaGetDevice(&dev));
+    FDAS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    float* sink = nullptr;
+    FDAS_CUDA(cudaMalloc(&sink, sizeof(float)));
+    const int iters = 4096, grid = sms * 8, block = 256;
+    cudaEvent_t e0, e1;
+    FDAS_CUDA(cudaEventCreate(&e0));
+    FDAS_CUDA(cudaEventCreate(&e1));
+    double best_ms = 1.0e30;
+    for (int rep = 0; rep < 5; rep++) {                       // rep 0 warms up; best of the rest (burst figure)
+        FDAS_CUDA(cudaEventRecord(e0, st));
+        k_ffma_peak<<<grid, block, 0, st>>>(sink, 0.999f, 1.0e-3f, iters);
+        FDAS_CUDA(cudaEventRecord(e1, st));
+        FDAS_CUDA(cudaEventSynchronize(e1));
+        FDAS_LAUNCH_CHECK();
+        float ms = 0.0f;
+        FDAS_CUDA(cudaEventElapsedTime(&ms, e0, e1));
+        if (rep > 0 && ms < best_ms) best_ms = ms;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    const double flops = 2.0 * 4.0 * PEAK_ACC * (double)iters * (double)grid * (double)block;
+    *out_tflops = flops / (best_ms * 1.0e-3) / 1.0e12;
+    if (out_ms) *out_ms = best_ms;
+    return FDAS_OK;
+}

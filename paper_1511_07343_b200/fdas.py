@@ -24,7 +24,7 @@ assert CAND_DTYPE.itemsize == 12
 
 EXPORTS = ["fdas_set_device", "fdas_plan_create", "fdas_plan_set_option", "fdas_plan_info",
            "fdas_build_templates", "fdas_get_templates", "fdas_spectrum", "fdas_correlate",
-           "fdas_harmsum", "fdas_candidates", "fdas_search_host", "fdas_threshold",
+           "fdas_harmsum", "fdas_candidates", "fdas_search_host", "fdas_threshold", "fdas_measure_fp32_tflops",
            "fdas_plan_destroy", "fdas_strerror"]
 
 
@@ -64,6 +64,7 @@ def lib():
         L.fdas_harmsum.argtypes = [vp, vp, i32, vp, vp, vp, u32, vp]
         L.fdas_candidates.argtypes = [vp, vp, f32, vp, vp, u32, vp]
         L.fdas_search_host.argtypes = [vp, vp, i32, i32, vp, vp, vp, u32, vp]
+        L.fdas_measure_fp32_tflops.argtypes = [C.POINTER(f64), C.POINTER(f64), vp]
         L.fdas_threshold.argtypes = [i32, f64]
         L.fdas_threshold.restype = f64
         L.fdas_plan_destroy.argtypes = [vp]
@@ -171,6 +172,13 @@ def fdas_search_host(plan, h_series: np.ndarray, max_harm, thresholds, capacity,
 
 def fdas_threshold(n_harm: int, pfa: float = 1e-6) -> float:
     return lib().fdas_threshold(int(n_harm), float(pfa))
+
+
+def fdas_measure_fp32_tflops(stream=None):
+    """(TFLOP/s, ms) of the FFMA-chain microbenchmark on the current device."""
+    tf, ms = C.c_double(), C.c_double()
+    _check(lib().fdas_measure_fp32_tflops(C.byref(tf), C.byref(ms), _stream(stream)), "fdas_measure_fp32_tflops")
+    return tf.value, ms.value
 
 
 def fdas_plan_destroy(plan):

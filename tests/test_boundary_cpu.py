@@ -25,7 +25,7 @@ def fdas():
 def declared_symbols():
     src = open(os.path.join(ROOT, "include", "fdas.h")).read()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(fdas_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(fdas_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_every_declared_symbol_is_exported(fdas):
