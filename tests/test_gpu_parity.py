@@ -353,3 +353,10 @@ def test_search_host_matches_device_calls(fdas):
     S, _ = oracle.spectrum(x)
     c_ref = oracle.candidates(oracle.correlate_direct(S, oracle.templates(cfg.z_max, cfg.dz, cfg.width)), 20.0)
     assert_cand_parity(h_c[0, :int(h_n[0])], c_ref, lambda h: 20.0)
+
+
+def test_fp32_peak_microbenchmark_is_sane(fdas):
+    """fdas_measure_fp32_tflops: a B200 must land between a quarter of and slightly above the nominal
+    148 SM x 128 lanes x 2 x 1.965 GHz = 74.4 TFLOP/s."""
+    tf, ms = fdas.fdas_measure_fp32_tflops()
+    assert 18.0 < tf < 85.0 and ms > 0.0
