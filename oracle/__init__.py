@@ -54,6 +54,8 @@ def lib():
         L.ofdas_candidates.restype = C.c_int64
         L.ofdas_harmsum.argtypes = [p, C.c_int32, C.c_int64, C.c_int32, C.c_int32, p, p, C.c_int64, p]
         L.ofdas_harmsum.restype = C.c_int64
+        L.ofdas_resample.argtypes = [p, C.c_int64, C.c_double, p]
+        L.ofdas_resample.restype = C.c_int
         L.ofdas_gamma_q.argtypes = [C.c_int32, C.c_double]
         L.ofdas_gamma_q.restype = C.c_double
         L.ofdas_threshold.argtypes = [C.c_int32, C.c_double]
@@ -171,6 +173,17 @@ def harmsum(P, max_harm: int, thresholds, bin0: int = 1, cap: int = 1 << 23, ret
     if n > cap:
         raise OverflowError("oracle candidate capacity %d < %d" % (cap, n))
     return (out[:n], S) if return_sums else out[:n]
+
+
+def resample(x, beta: float) -> np.ndarray:
+    """Time-domain acceleration trial (G23): nearest-sample resampling that undoes
+    the time offset beta (u^2 - u)."""
+    x = np.ascontiguousarray(x, dtype=np.float32)
+    y = np.empty_like(x)
+    rc = lib().ofdas_resample(_ptr(x), x.size, C.c_double(beta), _ptr(y))
+    if rc:
+        raise ValueError("ofdas_resample failed (%d)" % rc)
+    return y
 
 
 def gamma_q(H: int, T: float) -> float:

@@ -370,3 +370,34 @@ double ofdas_threshold(int32_t H, double pfa)
     }
     return 0.5 * (lo + hi);
 }
+
+/* ------------------------------------------------- time-domain resampling ---- */
+
+/* Time-domain acceleration trial ("resampling the time series according to a time
+ * offset caused by the constant acceleration, followed by a standard periodicity search"; the
+ * paper gives no formula: DESIGN.md reading G23).  With u = n/N in [0,1) the time offset of a
+ * constant acceleration, referred to mid-span, is beta (u^2 - u); a signal of mean frequency r0
+ * drifting z bins has phase r0 [u + (z/2r0)(u^2 - u)], so the trial beta = z/(2 r0) turns it into
+ * a pure tone at r0.  Output sample m (u' = m/N) takes the input sample nearest to the u that
+ * solves  u + beta (u^2 - u) = u',  u = 2u' / [(1-beta) + sqrt((1-beta)^2 + 4 beta u')]
+ * (the root that tends to u' as beta -> 0; no cancellation):
+ *   y[m] = x[ min(N-1, floor(u N + 1/2)) ].
+ * Each operation is a separately rounded IEEE fp64 operation (no contraction), in this order, so
+ * that the index can be reproduced bit for bit.  |beta| < 1/2 required (monotone map). */
+__attribute__((optimize("fp-contract=off")))
+int ofdas_resample(const float *x, int64_t N, double beta, float *y)
+{
+    if (N < 2 || !(beta > -0.5 && beta < 0.5)) return -1;
+    const double omb = 1.0 - beta, omb2 = omb * omb, fb = 4.0 * beta, dN = (double)N;
+    #pragma omp parallel for schedule(static)
+    for (int64_t m = 0; m < N; m++) {
+        double up = (double)m / dN;
+        double disc = omb2 + fb * up;
+        double u = (2.0 * up) / (omb + sqrt(disc));
+        int64_t n = (int64_t)floor(u * dN + 0.5);
+        if (n > N - 1) n = N - 1;
+        if (n < 0) n = 0;
+        y[m] = x[n];
+    }
+    return 0;
+}

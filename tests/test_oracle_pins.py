@@ -378,3 +378,44 @@ def test_all_zero_series_gives_zero_spectrum_G22():
     """Degenerate input (reading G22): mu = 0 -> S := 0, not 0/0."""
     S, mu = oracle.spectrum(np.zeros(1 << 10, np.float32))
     assert mu == 0.0 and not np.any(S)
+
+
+# ------------------------------------------------------------------ time-domain resampling (PAPER.md:17, G23)
+def test_resample_identity_and_nearest_sample_property():
+    N = 1 << 12
+    x = np.arange(N, dtype=np.float32)                  # y then holds the chosen source index itself
+    assert np.array_equal(oracle.resample(x, 0.0), x)
+    for beta in (0.3, -0.2, 1e-4):
+        n = oracle.resample(x, beta).astype(np.int64)
+        assert np.all(np.diff(n) >= 0) and n[0] == 0    # monotone map that starts at the first sample
+        # the chosen sample is the nearest to the exact solution of u + beta (u^2 - u) = m/N (evaluated in
+        # extended precision from the defining equation, not from the oracle's root formula)
+        m = np.arange(N, dtype=np.longdouble)
+        g = lambda nn: (nn / N + np.longdouble(beta) * ((nn / N) ** 2 - nn / N)) * N      # forward map, in samples
+        d0 = np.abs(g(n.astype(np.longdouble)) - m)
+        ok = n < N - 1                                   # the last sample is a clamp, not a nearest sample
+        assert np.all(d0[ok] <= np.abs(g(n + 1.0) - m)[ok] + 1e-9)
+        assert np.all(d0[n > 0] <= np.abs(g(n - 1.0) - m)[n > 0] + 1e-9)
+    with pytest.raises(ValueError):
+        oracle.resample(x, 0.5)
+
+
+def test_resample_turns_an_accelerated_sinusoid_into_a_tone():
+    """PAPER.md:17 in one number: a noise-free sinusoid of mean frequency r0 = 3000 drifting z = 24 bins,
+    resampled at beta = z/(2 r0), is a pure tone at bin r0: all of A^2 N/4 (here normalised by mu) comes back in
+    one bin, as for an unaccelerated tone, while the raw series leaves a few per cent there.  The FDAS plane
+    of the RAW series has the same power at (r0, z) -- the two searches cross-check each other."""
+    N, r0, z, A = 1 << 16, 3000, 24, 1.0
+    x = synth.make_series(N, 1, [synth.Signal(A, r0, z, 0.7)], noise=False)
+    S_raw, mu_raw = oracle.spectrum(x)
+    y = oracle.resample(x, z / (2.0 * r0))
+    S_y, mu_y = oracle.spectrum(y)
+    full = (A * N / 2) ** 2                              # |F_r0|^2 of a pure tone
+    p_y = abs(S_y[r0 - 1]) ** 2 * mu_y
+    assert p_y == pytest.approx(full, rel=0.02) and int(np.argmax(np.abs(S_y))) == r0 - 1
+    assert abs(S_raw[r0 - 1]) ** 2 * mu_raw < 0.2 * full
+    T = oracle.templates(24.0, 2.0, 64)
+    P = oracle.correlate_direct(S_raw, T, c0=r0 - 33, nc=64)
+    zi, c = np.unravel_index(np.argmax(P), P.shape)
+    assert (zi, c + r0 - 33) == (24, r0 - 1)             # row of z = +24, the column of bin r0
+    assert P[zi, c] * mu_raw == pytest.approx(full, rel=0.02)
