@@ -150,6 +150,17 @@ int fdas_harmsum(fdas_plan* plan, const float* d_plane, int32_t max_harm,
 int fdas_candidates(fdas_plan* plan, const float* d_plane, float threshold,
                     fdas_cand* d_cands, uint32_t* d_count, uint32_t capacity, void* stream);
 
+/* Time-domain acceleration trial ("resampling the time series according to a time offset
+ * caused by the constant acceleration, followed by a standard periodicity search"): with u = n/N the
+ * offset, referred to mid-span, is beta (u^2 - u), so beta = z/(2 r0) turns a signal of mean frequency r0
+ * drifting z bins into a tone at r0.  d_out[m] = d_series[min(N-1, floor(u N + 1/2))] with u the root
+ *   u = 2u' / [(1 - beta) + sqrt((1 - beta)^2 + 4 beta u')],  u' = m/N,   of  u + beta (u^2 - u) = u',
+ * the index being decided in fp64 with separately rounded operations.  d_series, d_out: float[N], distinct
+ * buffers, d_out 16-byte aligned; |beta| < 1/2 (FDAS_E_INVALID otherwise).  The periodicity search of d_out is
+ * fdas_spectrum followed by fdas_correlate / fdas_candidates on a plan with z_max = 0 (its single template
+ * is the delta, so the plane is |S|^2). */
+int fdas_resample(fdas_plan* plan, const float* d_series, double beta, float* d_out, void* stream);
+
 /* Host-buffer convenience path (what bench.py's "e2e" times): for each of n_batch series in
  * HOST memory, copy to the device, run spectrum -> correlate -> harmonic sum, and copy the
  * candidate list back.  max_harm = 0 selects the fused threshold mode of fdas_correlate

@@ -176,6 +176,14 @@ extern "C" int fdas_harmsum(fdas_plan* p, const float* d_plane, int32_t max_harm
     return fdas_launch_harmsum(p, d_plane, max_harm, h_thresholds, d_cands, d_count, capacity, (cudaStream_t)stream);
 }
 
+extern "C" int fdas_resample(fdas_plan* p, const float* d_series, double beta, float* d_out, void* stream)
+{
+    if (!p || !d_series || !d_out || d_series == d_out) return FDAS_E_INVALID;
+    if (!(beta > -0.5 && beta < 0.5)) return FDAS_E_INVALID;
+    if (misaligned(d_series, 4) || misaligned(d_out, 16)) return FDAS_E_INVALID;
+    return fdas_launch_resample(p, d_series, beta, d_out, (cudaStream_t)stream);
+}
+
 extern "C" int fdas_candidates(fdas_plan* p, const float* d_plane, float threshold, fdas_cand* d_cands,
                                uint32_t* d_count, uint32_t capacity, void* stream)
 {

@@ -50,6 +50,7 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
                           fdas_cand* d_cands, uint32_t* d_counts, uint32_t cap, cudaStream_t st);
 int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const float* h_thr,
                         fdas_cand* d_cands, uint32_t* d_count, uint32_t cap, cudaStream_t st);
+int fdas_launch_resample(fdas_plan* p, const float* d_series, double beta, float* d_out, cudaStream_t st);
 int fdas_launch_candidates(fdas_plan* p, const float* d_plane, float thr, fdas_cand* d_cands,
                            uint32_t* d_count, uint32_t cap, cudaStream_t st);
 

@@ -24,7 +24,7 @@ assert CAND_DTYPE.itemsize == 12
 
 EXPORTS = ["fdas_set_device", "fdas_plan_create", "fdas_plan_set_option", "fdas_plan_info",
            "fdas_build_templates", "fdas_get_templates", "fdas_spectrum", "fdas_correlate",
-           "fdas_harmsum", "fdas_candidates", "fdas_search_host", "fdas_threshold", "fdas_measure_fp32_tflops",
+           "fdas_harmsum", "fdas_candidates", "fdas_resample", "fdas_search_host", "fdas_threshold", "fdas_measure_fp32_tflops",
            "fdas_plan_destroy", "fdas_strerror"]
 
 
@@ -63,6 +63,7 @@ def lib():
         L.fdas_correlate.argtypes = [vp, vp, i32, vp, f32, vp, vp, u32, vp, vp]
         L.fdas_harmsum.argtypes = [vp, vp, i32, vp, vp, vp, u32, vp]
         L.fdas_candidates.argtypes = [vp, vp, f32, vp, vp, u32, vp]
+        L.fdas_resample.argtypes = [vp, vp, f64, vp, vp]
         L.fdas_search_host.argtypes = [vp, vp, i32, i32, vp, vp, vp, u32, vp]
         L.fdas_measure_fp32_tflops.argtypes = [C.POINTER(f64), C.POINTER(f64), vp]
         L.fdas_threshold.argtypes = [i32, f64]
@@ -145,6 +146,10 @@ def fdas_harmsum(plan, d_plane, max_harm, thresholds, d_cands, d_count, capacity
 def fdas_candidates(plan, d_plane, threshold, d_cands, d_count, capacity, stream=None):
     _check(lib().fdas_candidates(plan, _dptr(d_plane), float(threshold), _dptr(d_cands), _dptr(d_count),
                                  int(capacity), _stream(stream)), "fdas_candidates")
+
+
+def fdas_resample(plan, d_series, beta, d_out, stream=None):
+    _check(lib().fdas_resample(plan, _dptr(d_series), float(beta), _dptr(d_out), _stream(stream)), "fdas_resample")
 
 
 def fdas_search_host(plan, h_series: np.ndarray, max_harm, thresholds, capacity, h_cands=None, h_counts=None,
@@ -253,6 +258,12 @@ class Plan:
 
     def candidates(self, d_plane, threshold, cands, capacity, stream=None):
         fdas_candidates(self.handle, d_plane, threshold, cands[0], cands[1], capacity, stream)
+
+    def resample(self, d_series, beta, d_out=None, stream=None):
+        if d_out is None:
+            d_out = torch.empty_like(d_series)
+        fdas_resample(self.handle, d_series, beta, d_out, stream)
+        return d_out
 
     def search_host(self, h_series, max_harm, thr, capacity, h_cands=None, h_counts=None, stream=None):
         return fdas_search_host(self.handle, h_series, max_harm, thr, capacity, h_cands, h_counts, stream)

@@ -108,6 +108,12 @@ static inline void sincospi(double x, double* s, double* c)
     *s = sin(M_PI * r);
     *c = cos(M_PI * r);
 }
+// separately rounded fp64 operations (the emu build has no FMA contraction: plain x86-64, -ffp-contract=off)
+static inline double __dadd_rn(double a, double b) { volatile double r = a + b; return r; }
+static inline double __dsub_rn(double a, double b) { volatile double r = a - b; return r; }
+static inline double __dmul_rn(double a, double b) { volatile double r = a * b; return r; }
+static inline double __ddiv_rn(double a, double b) { volatile double r = a / b; return r; }
+static inline double __dsqrt_rn(double a) { volatile double r = sqrt(a); return r; }
 static inline int min(int a, int b) { return a < b ? a : b; }
 static inline int max(int a, int b) { return a > b ? a : b; }
 static inline long long min(long long a, long long b) { return a < b ? a : b; }

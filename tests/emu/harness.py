@@ -101,6 +101,12 @@ class Plan:
         n = int(d_n.np()[0])
         return d_c.np()[:min(n, cap)].copy(), n
 
+    def resample(self, x, beta):
+        d_x = to_dev(np.asarray(x, np.float32))
+        d_y = DevBuf(d_x.shape, np.float32)
+        fdas.fdas_resample(self.handle, d_x, beta, d_y)
+        return d_y.np().copy()
+
     def candidates(self, d_P, thr, cap):
         d_c = DevBuf(cap, fdas.CAND_DTYPE)
         d_n = DevBuf(1, np.uint32)

@@ -159,6 +159,35 @@ def test_pulse_train_is_found_by_the_harmonic_sum(emu):
     assert (int(best["nharm"]), int(best["col"]), int(best["zi"])) == (8, r0 * nh - 1, 8 + z0 * nh)
 
 
+@pytest.mark.parametrize("beta", [0.0, 0.004, -0.3, 0.49])
+def test_resample_is_bit_exact(emu, beta):
+    N = 1 << 13
+    x = synth.make_series(N, 31)
+    plan = emu.Plan(N, 0.0, 2.0, 2, 2048, quad_points=64)
+    assert np.array_equal(plan.resample(x, beta), oracle.resample(x, beta))
+    plan.close()
+
+
+def test_time_domain_trial_end_to_end(emu):
+    """PAPER.md:17 through the CUDA path: resample at beta = z/(2 r0), spectrum, |S|^2 by the z_max = 0 plan
+    (one delta template), candidates -- the accelerated sinusoid comes back as a tone at r0."""
+    N, r0, z = 1 << 14, 1500, 12.0
+    x = synth.make_series(N, 32, [synth.Signal(0.2, r0, z, 0.3)])
+    plan = emu.Plan(N, 0.0, 2.0, 2, 2048, quad_points=64)
+    y = plan.resample(x, z / (2.0 * r0))
+    assert np.array_equal(y, oracle.resample(x, z / (2.0 * r0)))
+    d_S, _ = plan.spectrum(y)
+    d_P, d_c, d_n = plan.correlate(d_S, True, 40.0, 64)
+    S_ref, _ = oracle.spectrum(y)
+    power_ok(d_P.np()[0, 0], np.abs(S_ref) ** 2)                      # the delta template: plane row = |S|^2
+    c = d_c.np()[0, :int(d_n.np()[0])]
+    assert len(c) >= 1 and int(c[np.argmax(c["power"])]["col"]) == r0 - 1
+    d_S0, _ = plan.spectrum(x)                                        # without the resampling the tone is smeared
+    d_P0, _, _ = plan.correlate(d_S0, True)
+    assert d_P0.np().max() < 0.5 * d_P.np().max()
+    plan.close()
+
+
 def test_fused_batch(emu):
     small = synth.small_config(1 << 13, 8.0, 2.0, 64, 2048, n_dm=5, n_sig=1, index=33, amp=0.3)
     xs = np.stack([small.series(d) for d in range(5)])
