@@ -231,6 +231,7 @@ def run_ours(args):
     stage_all = np.array([[m[j].elapsed_time(m[j + 1]) for j in range(3)] for m in marks])
     stage = stage_all.mean(axis=0)
     fp32_measured, _ = fdas.fdas_measure_fp32_tflops()       # FFMA-chain microbenchmark (untimed region)
+    fp32_packed, _ = fdas.fdas_measure_fp32_tflops(packed=True)
     n_found = int(cands[1][0])
 
     # BASELINE.json configs[3] (streaming batch, plane not stored, threshold fused into the segment kernel):
@@ -346,7 +347,8 @@ def run_ours(args):
         "stage_ms": {"spectrum": spec_ms, "correlate": corr_ms, "harmsum": hs_ms},
         "stage_ms_median": dict(zip(("spectrum", "correlate", "harmsum"), (float(v) for v in np.median(stage_all, axis=0)))),
         "stage_ms_min": dict(zip(("spectrum", "correlate", "harmsum"), (float(v) for v in stage_all.min(axis=0)))),
-        "fp32_peak": {"nominal_tflops": FP32_PEAK_TFLOPS, "measured_ffma_tflops": fp32_measured},
+        "fp32_peak": {"nominal_tflops": FP32_PEAK_TFLOPS, "measured_ffma_tflops": fp32_measured,
+                      "measured_ffma2_tflops": fp32_packed},
         "fft_correlation_roofline": {"ms_at_roofline": t_roof_ms, "ms_measured": spec_ms + corr_ms,
                                      "frac": t_roof_ms / (spec_ms + corr_ms),
                                      "dm_trials_per_s_without_harmsum": world * 1e3 / (spec_ms + corr_ms)},

@@ -179,7 +179,9 @@ double fdas_threshold(int32_t n_harm, double pfa);
 
 /* Measurement aid: the FP32 fused-multiply-add rate of the current device in
  * TFLOP/s, from a kernel of independent FFMA chains (a <- a*x + y) on every SM, best of 4 timed
- * launches with CUDA events on `stream`; *out_ms (may be NULL) receives that launch's duration.
+ * launches with CUDA events on `stream`; *out_ms (may be NULL) receives that launch's duration, and a
+ * NEGATIVE *out_ms on entry selects the same chains written with the packed f32x2 instruction of sm_100
+ * (FFMA2, two FMAs per lane and issue slot) so that both rates can be reported.
  * bench.py reports the fused correlate kernel against this measured peak as well as the nominal one.
  * Synchronises `stream`; allocates and frees 4 bytes of device memory.  Not part of the search path. */
 int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, void* stream);

@@ -83,7 +83,9 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
             }
         }
     }
-    float v[HS_CPT][HMAX];
+    static_assert(HS_CPT % 2 == 0, "cells are summed in pairs (packed f32x2 adds)");
+    float2 v[HS_CPT / 2][HMAX];                                       // .x, .y = cells 2jj, 2jj+1 of the lane
+#define HS_V(j, i) (((j) & 1) ? v[(j) >> 1][i].y : v[(j) >> 1][i].x)
     for (int zi = r_begin; zi < r_end; zi++) {
         const int zeta = zi - zc;
         const int t = abs(zeta) * my_h + (my_H >> 1), fr = t & (my_H - 1);
@@ -93,7 +95,7 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
         {
             const float* src = plane + idx[0];
 #pragma unroll
-            for (int j = 0; j < HS_CPT; j++) v[j][0] = (!CHECK || (okmask >> j & 1)) ? __ldcs(src + 32 * j) : 0.0f;
+            for (int j = 0; j < HS_CPT; j++) HS_V(j, 0) = (!CHECK || (okmask >> j & 1)) ? __ldcs(src + 32 * j) : 0.0f;
             idx[0] += n_cols;
         }
 #pragma unroll
@@ -108,32 +110,38 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
                     const int dk = (32 * h) >> st;                     // exact: 32 h / H
 #pragma unroll
                     for (int j = 0; j < HS_CPT; j++)
-                        v[j][slot] = (!CHECK || (okmask >> (slot * HS_CPT + j) & 1)) ? __ldg(src + dk * j) : 0.0f;
+                        HS_V(j, slot) = (!CHECK || (okmask >> (slot * HS_CPT + j) & 1)) ? __ldg(src + dk * j) : 0.0f;
                 }
             }
         }
 #pragma unroll
-        for (int j = 0; j < HS_CPT; j++) {
-            // the stage sums, and ONE branch for the (rare) cell that passes any threshold
-            float sum[NST];
-            float acc = v[j][0];
+        for (int jj = 0; jj < HS_CPT / 2; jj++) {
+            // the stage sums of two cells at a time (FADD2: one issue slot for both), and ONE branch for the
+            // (rare) cell that passes any threshold
+            float2 sum[NST];
+            float2 acc = v[jj][0];
             sum[0] = acc;
-            bool any = acc > thr.t[0];
+            bool any = acc.x > thr.t[0] || acc.y > thr.t[0];
 #pragma unroll
             for (int st = 1; st < NST; st++) {
                 const int H = 1 << st;
 #pragma unroll
-                for (int i = H >> 1; i < H; i++) acc += v[j][i];
+                for (int i = H >> 1; i < H; i++) acc = __fadd2_rn(acc, v[jj][i]);
                 sum[st] = acc;
-                any = any || acc > thr.t[st];
+                any = any || acc.x > thr.t[st] || acc.y > thr.t[st];
             }
-            if (any && (!CHECK || (okmask >> j & 1))) {
+            if (any) {
 #pragma unroll
-                for (int st = 0; st < NST; st++)
-                    if (sum[st] > thr.t[st]) push_cand_hs(cands, count, cap, col0 + 32 * j, zi, 1 << st, sum[st]);
+                for (int st = 0; st < NST; st++) {
+                    if (sum[st].x > thr.t[st] && (!CHECK || (okmask >> (2 * jj) & 1)))
+                        push_cand_hs(cands, count, cap, col0 + 32 * (2 * jj), zi, 1 << st, sum[st].x);
+                    if (sum[st].y > thr.t[st] && (!CHECK || (okmask >> (2 * jj + 1) & 1)))
+                        push_cand_hs(cands, count, cap, col0 + 32 * (2 * jj + 1), zi, 1 << st, sum[st].y);
+                }
             }
         }
     }
+#undef HS_V
 }
 
 // Tile order.  The stretch (k, zeta) -> (k h/H, zeta h/H) moves a cell along the ray through the origin of

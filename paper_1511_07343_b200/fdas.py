@@ -179,9 +179,9 @@ def fdas_threshold(n_harm: int, pfa: float = 1e-6) -> float:
     return lib().fdas_threshold(int(n_harm), float(pfa))
 
 
-def fdas_measure_fp32_tflops(stream=None):
-    """(TFLOP/s, ms) of the FFMA-chain microbenchmark on the current device."""
-    tf, ms = C.c_double(), C.c_double()
+def fdas_measure_fp32_tflops(stream=None, packed=False):
+    """(TFLOP/s, ms) of the FFMA-chain microbenchmark on the current device (packed: FFMA2 chains)."""
+    tf, ms = C.c_double(), C.c_double(-1.0 if packed else 0.0)
     _check(lib().fdas_measure_fp32_tflops(C.byref(tf), C.byref(ms), _stream(stream)), "fdas_measure_fp32_tflops")
     return tf.value, ms.value
 
