@@ -389,3 +389,5 @@ def test_fp32_peak_microbenchmark_is_sane(fdas):
     148 SM x 128 lanes x 2 x 1.965 GHz = 74.4 TFLOP/s."""
     tf, ms = fdas.fdas_measure_fp32_tflops()
     assert 18.0 < tf < 85.0 and ms > 0.0
+    tf2, _ = fdas.fdas_measure_fp32_tflops(packed=True)               # FFMA2 chains: same lanes, half the issue slots
+    assert 18.0 < tf2 < 170.0
