@@ -203,6 +203,8 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
 //     8 LDS.128 (quarter-warp bank pattern 4 lo + 4 j: conflict-free);
 //   * pass 3 owns the ADJACENT outputs p = 2 tid, 2 tid + 1: 8 LDS.128 from exchange 2, and for
 //     integer-bin planes 8-byte stores of two neighbouring columns;
+//   * PK: the butterflies use the packed f32x2 instructions of sm_100 (FFMA2/FADD2/FMUL2, fdas_regfft.cuh): the
+//     same operations per component in the same order (bit-identical planes), ~15 % fewer issue slots;
 //   * FAST (launched when step is a multiple of 256): a full segment keeps exactly t3 < step/256
 //     for every thread, so its stores are unpredicated and the butterflies feeding the discarded
 //     t3 = 7 outputs are dead code; the ragged last segment takes the predicated path.
@@ -213,7 +215,7 @@ constexpr int V2_BUF = 8 * V2_PITCH3;
 // 8 LDS.128 from exchange 2, two 8-point DITs over k3, |.|^2, store / threshold.
 // FULL (CTA-uniform): every thread keeps exactly t3 < NKEEP, so nothing is predicated and the work
 // feeding t3 >= NKEEP is dead code; otherwise t3 < nv (ragged last segment, or step not a multiple of 256).
-template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool FULL>
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool FULL, bool PK>
 __device__ __forceinline__ void v2_pass3(const float2* buf, const float2* tw_a, const float2* tw_b, int tid,
                                          float* prow, int nv, fdas_cand* cands, uint32_t* counts, uint32_t cap,
                                          float thr, int col0, int zi)
@@ -225,8 +227,8 @@ __device__ __forceinline__ void v2_pass3(const float2* buf, const float2* tw_a, 
         u0[bitrev(k3, 3)] = make_float2(q.x, q.y);
         u1[bitrev(k3, 3)] = make_float2(q.z, q.w);
     }
-    dit_tw<8>(u0, tw_a);
-    dit_tw<8>(u1, tw_b);
+    dit_tw<8, PK>(u0, tw_a);
+    dit_tw<8, PK>(u1, tw_b);
     float pa[8], pb[8];
     float mx = 0.0f;                                   // largest kept power of this thread (fused threshold: one test)
 #pragma unroll
@@ -250,7 +252,7 @@ __device__ __forceinline__ void v2_pass3(const float2* buf, const float2* tw_a, 
     }
 }
 
-template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP>
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK>
 __global__ void __launch_bounds__(V1_THREADS, 3)
 k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
                     fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
@@ -328,10 +330,11 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
     for (int t = t_begin; t < t_end; t++) {
         float2* buf = sm + ((t - t_begin) & 1) * V2_BUF;
         float2 v[16];
-        mul_first_stage16(v, X, w4);                                             // X W and stage 1
-        dit_const_stage<16, +1, 2>(v);                                           // pass 1: k1 -> t1
-        dit_const_stage<16, +1, 3>(v);
-        dit_const_stage<16, +1, 4>(v);
+        if (PK) mul_first_stage16_pk(v, X, w4);                                  // X W and stage 1
+        else mul_first_stage16(v, X, w4);
+        dit_const_stage<16, +1, 2, PK>(v);                                       // pass 1: k1 -> t1
+        dit_const_stage<16, +1, 3, PK>(v);
+        dit_const_stage<16, +1, 4, PK>(v);
 #pragma unroll
         for (int t1 = 0; t1 < 16; t1++) buf[lo + 18 * t1 + V2_PITCH3 * k3A] = v[t1];
         __syncwarp();
@@ -344,7 +347,7 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
                 v[bitrev(2 * j + 1, 4)] = make_float2(q.z, q.w);
             }
         }
-        dit_tw<16>(v, tw2);                                                      // pass 2: k2 -> t2
+        dit_tw<16, PK>(v, tw2);                                                  // pass 2: k2 -> t2
         __syncwarp();
 #pragma unroll
         for (int t2 = 0; t2 < 16; t2++) buf[lo + 16 * t2 + V2_PITCH3 * k3A] = v[t2];
@@ -357,9 +360,9 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
         if (HAS_PLANE && NSET == 1) prow1 += n_cols;
         const int col0 = (c0 + 2 * tid) * nset + s;
         if (full)                                                                // pass 3: k3 -> t3
-            v2_pass3<HAS_PLANE, HAS_CANDS, NSET, NKEEP, true>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
+            v2_pass3<HAS_PLANE, HAS_CANDS, NSET, NKEEP, true, PK>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
         else
-            v2_pass3<HAS_PLANE, HAS_CANDS, NSET, 8, false>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
+            v2_pass3<HAS_PLANE, HAS_CANDS, NSET, 8, false, PK>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
     }
 }
 
@@ -402,13 +405,21 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
         else if (d_plane) K<true, false, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);      \
         else K<false, true, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS)
         static const bool use_v1 = getenv("FDAS_CORRELATE_V1") != nullptr;
+        static const bool scalar = getenv("FDAS_CORRELATE_SCALAR") != nullptr;     // v2 with scalar FFMA butterflies
+        const bool keep7 = p->step == 7 * 256;                    // m = 256: full segments keep t3 < 7 exactly
+#define FDAS_V2_LAUNCH(NS)                                                                                        \
+        if (keep7 && !scalar) { FDAS_V1_LAUNCH(k_correlate_2048_v2, NS, 7, true); }                               \
+        else if (keep7) { FDAS_V1_LAUNCH(k_correlate_2048_v2, NS, 7, false); }                                    \
+        else if (!scalar) { FDAS_V1_LAUNCH(k_correlate_2048_v2, NS, 8, true); }                                   \
+        else { FDAS_V1_LAUNCH(k_correlate_2048_v2, NS, 8, false); }
         if (use_v1) {
             if (p->nset == 1) { FDAS_V1_LAUNCH(k_correlate_2048, 1); } else { FDAS_V1_LAUNCH(k_correlate_2048, 2); }
-        } else if (p->step == 7 * 256) {                          // m = 256: full segments keep t3 < 7 exactly
-            if (p->nset == 1) { FDAS_V1_LAUNCH(k_correlate_2048_v2, 1, 7); } else { FDAS_V1_LAUNCH(k_correlate_2048_v2, 2, 7); }
+        } else if (p->nset == 1) {
+            FDAS_V2_LAUNCH(1)
         } else {
-            if (p->nset == 1) { FDAS_V1_LAUNCH(k_correlate_2048_v2, 1, 8); } else { FDAS_V1_LAUNCH(k_correlate_2048_v2, 2, 8); }
+            FDAS_V2_LAUNCH(2)
         }
+#undef FDAS_V2_LAUNCH
 #undef FDAS_V1_LAUNCH
 #undef FDAS_V1_ARGS
         FDAS_LAUNCH_CHECK();

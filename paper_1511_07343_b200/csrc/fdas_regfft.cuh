@@ -67,8 +67,41 @@ __device__ __forceinline__ void bfly_pmi(float2& a, float2& b)
     a = make_float2(a.x + t.x, a.y + t.y);
 }
 
+// ---- the same butterflies with the packed f32x2 instructions of sm_100 (FFMA2 / FADD2 / FMUL2): a complex
+// value is a natural (re, im) register pair, the twiddle components are broadcast (the .F32 operand form),
+// i*b = (-b.y, b.x) is an operand swizzle + sign pattern, so a +- tau b is 3 issue slots instead of 6 and
+// every component sees exactly the operations, in the order, of the scalar version (bit-identical results).
+__device__ __forceinline__ float2 f2(float x, float y) { return make_float2(x, y); }
+__device__ __forceinline__ void bfly_pk(float2& a, float2& b, float c, float s)
+{
+    const float2 t = __ffma2_rn(f2(c, c), b, a);                               // a + c b
+    const float2 o0 = __ffma2_rn(f2(s, s), f2(-b.y, b.x), t);                  // + s (i b)
+    b = __ffma2_rn(f2(2.0f, 2.0f), a, f2(-o0.x, -o0.y));
+    a = o0;
+}
+__device__ __forceinline__ void bfly_i_pk(float2& a, float2& b, float c, float s)     // tau = i (c, s)
+{
+    const float2 t = __ffma2_rn(f2(-s, -s), b, a);
+    const float2 o0 = __ffma2_rn(f2(c, c), f2(-b.y, b.x), t);
+    b = __ffma2_rn(f2(2.0f, 2.0f), a, f2(-o0.x, -o0.y));
+    a = o0;
+}
+__device__ __forceinline__ void bfly_1_pk(float2& a, float2& b)
+{
+    const float2 t = b;
+    b = __fadd2_rn(a, f2(-t.x, -t.y));
+    a = __fadd2_rn(a, t);
+}
+template <int SIGN>
+__device__ __forceinline__ void bfly_pmi_pk(float2& a, float2& b)
+{
+    const float2 t = (SIGN > 0) ? f2(-b.y, b.x) : f2(b.y, -b.x);
+    b = __fadd2_rn(a, f2(-t.x, -t.y));
+    a = __fadd2_rn(a, t);
+}
+
 // one DIT stage (span = 2^ST) with constant twiddles omega_span^q
-template <int R, int SIGN, int ST>
+template <int R, int SIGN, int ST, bool PK = false>
 __device__ __forceinline__ void dit_const_stage(float2* v)
 {
     constexpr int span = 1 << ST, half = span >> 1;
@@ -77,9 +110,15 @@ __device__ __forceinline__ void dit_const_stage(float2* v)
 #pragma unroll
         for (int q = 0; q < half; q++) {
             const int e = q * (16 / span);           // omega_span^q = exp(SIGN 2 pi i e / 16), e in [0, 8)
-            if (e == 0) bfly_1(v[b + q], v[b + q + half]);
-            else if (e == 4) bfly_pmi<SIGN>(v[b + q], v[b + q + half]);
-            else bfly(v[b + q], v[b + q + half], cos16(e), SIGN > 0 ? sin16(e) : -sin16(e));
+            if (PK) {
+                if (e == 0) bfly_1_pk(v[b + q], v[b + q + half]);
+                else if (e == 4) bfly_pmi_pk<SIGN>(v[b + q], v[b + q + half]);
+                else bfly_pk(v[b + q], v[b + q + half], cos16(e), SIGN > 0 ? sin16(e) : -sin16(e));
+            } else {
+                if (e == 0) bfly_1(v[b + q], v[b + q + half]);
+                else if (e == 4) bfly_pmi<SIGN>(v[b + q], v[b + q + half]);
+                else bfly(v[b + q], v[b + q + half], cos16(e), SIGN > 0 ? sin16(e) : -sin16(e));
+            }
         }
     }
 }
@@ -116,7 +155,26 @@ __device__ __forceinline__ void mul_first_stage16(float2* v, const float2* X, co
     }
 }
 
-template <int R, int ST>
+// mul_first_stage16 with packed instructions (same operations per component, in the same order)
+__device__ __forceinline__ void mul_first_stage16_pk(float2* v, const float2* X, const float4* w4)
+{
+#pragma unroll
+    for (int k1 = 0; k1 < 8; k1++) {
+        const float4 wa4 = w4[k1 >> 1], wb4 = w4[(k1 >> 1) + 4];
+        const float2 wa = (k1 & 1) ? f2(wa4.z, wa4.w) : f2(wa4.x, wa4.y);
+        const float2 wb = (k1 & 1) ? f2(wb4.z, wb4.w) : f2(wb4.x, wb4.y);
+        const float2 a = X[k1], b = X[k1 + 8];
+        const float2 m = __fmul2_rn(f2(a.y, a.y), f2(-wa.y, wa.x));            // (-a.y wa.y, a.y wa.x)
+        const float2 pp = __ffma2_rn(f2(a.x, a.x), wa, m);                      // p = X_a W_a
+        const float2 t = __ffma2_rn(f2(b.x, b.x), wb, pp);
+        const float2 o0 = __ffma2_rn(f2(b.y, b.y), f2(-wb.y, wb.x), t);         // p + X_b W_b
+        const int o = bitrev(k1, 4);
+        v[o] = o0;
+        v[o + 1] = __ffma2_rn(f2(2.0f, 2.0f), pp, f2(-o0.x, -o0.y));
+    }
+}
+
+template <int R, int ST, bool PK = false>
 __device__ __forceinline__ void dit_tw_stage(float2* v, const float2* tw)
 {
     constexpr int span = 1 << ST, half = span >> 1;
@@ -126,8 +184,13 @@ __device__ __forceinline__ void dit_tw_stage(float2* v, const float2* tw)
     for (int b = 0; b < R; b += span) {
 #pragma unroll
         for (int q = 0; q < half; q++) {
-            if (q < nind) bfly(v[b + q], v[b + q + half], tw[base + q].x, tw[base + q].y);
-            else bfly_i(v[b + q], v[b + q + half], tw[base + q - nind].x, tw[base + q - nind].y);
+            if (PK) {
+                if (q < nind) bfly_pk(v[b + q], v[b + q + half], tw[base + q].x, tw[base + q].y);
+                else bfly_i_pk(v[b + q], v[b + q + half], tw[base + q - nind].x, tw[base + q - nind].y);
+            } else {
+                if (q < nind) bfly(v[b + q], v[b + q + half], tw[base + q].x, tw[base + q].y);
+                else bfly_i(v[b + q], v[b + q + half], tw[base + q - nind].x, tw[base + q - nind].y);
+            }
         }
     }
 }
@@ -135,13 +198,13 @@ __device__ __forceinline__ void dit_tw_stage(float2* v, const float2* tw)
 // DIT on R points with inter-pass twiddle base w (inverse sign, SIGN = +1).
 // tw[] holds, for stage span = 2, 4, 8, 16: w^(R/span) * omega_span^q for q in [0, max(1, span/4)):
 //   index 0: span 2;  1: span 4;  2..3: span 8;  4..7: span 16.   (the other q are i * these)
-template <int R>
+template <int R, bool PK = false>
 __device__ __forceinline__ void dit_tw(float2* v, const float2* tw)
 {
-    dit_tw_stage<R, 1>(v, tw);
-    dit_tw_stage<R, 2>(v, tw);
-    dit_tw_stage<R, 3>(v, tw);
-    if constexpr (R >= 16) dit_tw_stage<R, 4>(v, tw);
+    dit_tw_stage<R, 1, PK>(v, tw);
+    dit_tw_stage<R, 2, PK>(v, tw);
+    dit_tw_stage<R, 3, PK>(v, tw);
+    if constexpr (R >= 16) dit_tw_stage<R, 4, PK>(v, tw);
 }
 
 // Fill tw[] for dit_tw<R>: w = exp(2 pi i num / den)  (num/den exact in fp32).
