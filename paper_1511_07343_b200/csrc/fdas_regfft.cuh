@@ -72,17 +72,20 @@ __device__ __forceinline__ void bfly_pmi(float2& a, float2& b)
 // i*b = (-b.y, b.x) is an operand swizzle + sign pattern, so a +- tau b is 3 issue slots instead of 6 and
 // every component sees exactly the operations, in the order, of the scalar version (bit-identical results).
 __device__ __forceinline__ float2 f2(float x, float y) { return make_float2(x, y); }
+// -x by flipping the sign bit on the integer pipe: building i*b = (-b.y, b.x) then costs the FMA pipe nothing
+// (a float negation would be an FADD there); exact, so results do not change.
+__device__ __forceinline__ float negi(float x) { return __int_as_float(__float_as_int(x) ^ 0x80000000); }
 __device__ __forceinline__ void bfly_pk(float2& a, float2& b, float c, float s)
 {
     const float2 t = __ffma2_rn(f2(c, c), b, a);                               // a + c b
-    const float2 o0 = __ffma2_rn(f2(s, s), f2(-b.y, b.x), t);                  // + s (i b)
+    const float2 o0 = __ffma2_rn(f2(s, s), f2(negi(b.y), b.x), t);             // + s (i b)
     b = __ffma2_rn(f2(2.0f, 2.0f), a, f2(-o0.x, -o0.y));
     a = o0;
 }
 __device__ __forceinline__ void bfly_i_pk(float2& a, float2& b, float c, float s)     // tau = i (c, s)
 {
     const float2 t = __ffma2_rn(f2(-s, -s), b, a);
-    const float2 o0 = __ffma2_rn(f2(c, c), f2(-b.y, b.x), t);
+    const float2 o0 = __ffma2_rn(f2(c, c), f2(negi(b.y), b.x), t);
     b = __ffma2_rn(f2(2.0f, 2.0f), a, f2(-o0.x, -o0.y));
     a = o0;
 }
@@ -164,10 +167,10 @@ __device__ __forceinline__ void mul_first_stage16_pk(float2* v, const float2* X,
         const float2 wa = (k1 & 1) ? f2(wa4.z, wa4.w) : f2(wa4.x, wa4.y);
         const float2 wb = (k1 & 1) ? f2(wb4.z, wb4.w) : f2(wb4.x, wb4.y);
         const float2 a = X[k1], b = X[k1 + 8];
-        const float2 m = __fmul2_rn(f2(a.y, a.y), f2(-wa.y, wa.x));            // (-a.y wa.y, a.y wa.x)
+        const float2 m = __fmul2_rn(f2(a.y, a.y), f2(negi(wa.y), wa.x));       // (-a.y wa.y, a.y wa.x)
         const float2 pp = __ffma2_rn(f2(a.x, a.x), wa, m);                      // p = X_a W_a
         const float2 t = __ffma2_rn(f2(b.x, b.x), wb, pp);
-        const float2 o0 = __ffma2_rn(f2(b.y, b.y), f2(-wb.y, wb.x), t);         // p + X_b W_b
+        const float2 o0 = __ffma2_rn(f2(b.y, b.y), f2(negi(wb.y), wb.x), t);    // p + X_b W_b
         const int o = bitrev(k1, 4);
         v[o] = o0;
         v[o + 1] = __ffma2_rn(f2(2.0f, 2.0f), pp, f2(-o0.x, -o0.y));

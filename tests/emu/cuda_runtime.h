@@ -115,6 +115,8 @@ static inline double __dmul_rn(double a, double b) { volatile double r = a * b; 
 static inline double __ddiv_rn(double a, double b) { volatile double r = a / b; return r; }
 static inline double __dsqrt_rn(double a) { volatile double r = sqrt(a); return r; }
 static inline float2 __ffma2_rn(float2 a, float2 b, float2 c) { return float2{fmaf(a.x, b.x, c.x), fmaf(a.y, b.y, c.y)}; }
+static inline int __float_as_int(float x) { int i; memcpy(&i, &x, 4); return i; }
+static inline float __int_as_float(int i) { float x; memcpy(&x, &i, 4); return x; }
 static inline float2 __fmul2_rn(float2 a, float2 b) { return float2{a.x * b.x, a.y * b.y}; }
 static inline float2 __fadd2_rn(float2 a, float2 b) { return float2{a.x + b.x, a.y + b.y}; }
 static inline int min(int a, int b) { return a < b ? a : b; }
