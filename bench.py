@@ -161,6 +161,57 @@ def run_sweep(args):
                       "note": "the plane (n_t x 2^22 fp32) is written every step: larger than L2 from 8 templates on"}))
 
 
+def run_ab(args):
+    """--ab: time the kernel variants kept for tuning, in one process (the library reads its FDAS_* switches
+    at every call): fused correlate v1 / v2 scalar / v2 packed, harmonic sum for several sector counts and
+    the 128-column variant.  One JSON line; nothing here is a bench value."""
+    import torch
+    from paper_1511_07343_b200 import build as fbuild, fdas, synth
+    torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
+    fbuild.build()
+    cfg = synth.config(2)
+    plan = fdas.Plan(cfg.n_samples, cfg.z_max, cfg.dz, cfg.width, cfg.seg_len)
+    d_x = torch.from_numpy(cfg.series()).cuda().view(1, -1)
+    d_spec, d_mu = plan.spectrum(d_x)
+    d_plane = plan.empty_plane(1)
+    cap = 1 << 22
+    cands = plan.empty_cands(cap)
+    thr = fdas.thresholds(16)
+    stream = torch.cuda.current_stream()
+
+    def timed(fn, env):
+        keys = [k for k in os.environ if k.startswith("FDAS_")]
+        for k in keys:
+            del os.environ[k]
+        os.environ.update(env)
+        for _ in range(3):
+            fn()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        for _ in range(args.steps):
+            fn()
+        e1.record(stream)
+        torch.cuda.synchronize()
+        for k in env:
+            del os.environ[k]
+        return e0.elapsed_time(e1) / args.steps
+
+    corr = lambda: fdas.fdas_correlate(plan.handle, d_spec, 1, d_plane, 0.0, None, None, 0)
+    hs = lambda: fdas.fdas_harmsum(plan.handle, d_plane[0], 16, thr, cands[0], cands[1], cap)
+    out = {"correlate_ms": {}, "harmsum_ms": {}, "steps": args.steps}
+    for name, env in (("v2_packed", {}), ("v2_scalar", {"FDAS_CORRELATE_SCALAR": "1"}), ("v1", {"FDAS_CORRELATE_V1": "1"}),
+                      ("v2_packed_4chunks", {"FDAS_T_CHUNKS": "4"}), ("v2_packed_2chunks", {"FDAS_T_CHUNKS": "2"})):
+        out["correlate_ms"][name] = timed(corr, env)
+    corr()
+    for name, env in (("S16", {}), ("S1", {"FDAS_HS_SECTORS": "1"}), ("S8", {"FDAS_HS_SECTORS": "8"}),
+                      ("S32", {"FDAS_HS_SECTORS": "32"}), ("S16_rows2", {"FDAS_HS_ROWS": "2"}),
+                      ("S16_128col", {"FDAS_HS_VARIANT": "1"}), ("S32_128col", {"FDAS_HS_VARIANT": "1", "FDAS_HS_SECTORS": "32"})):
+        out["harmsum_ms"][name] = timed(hs, env)
+        out.setdefault("harmsum_candidates", {})[name] = int(cands[1][0])
+    print(json.dumps(out))
+
+
 def run_ours(args):
     import numpy as np
     import torch
@@ -384,11 +435,14 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu", action="store_true", help="skip the cpu_baseline leg")
+    ap.add_argument("--ab", action="store_true", help="time the kernel variants kept for tuning instead")
     ap.add_argument("--sweep-templates", action="store_true",
                     help="time spectrum + correlate against the number of templates (PAPER.md Fig. 2) instead")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
-    if args.sweep_templates:
+    if args.ab:
+        run_ab(args)
+    elif args.sweep_templates:
         run_sweep(args)
     elif args.impl == "reference":
         run_reference(args)

@@ -391,9 +391,9 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
                           fdas_cand* d_cands, uint32_t* d_counts, uint32_t cap, cudaStream_t st)
 {
     if (d_cands) FDAS_CUDA(cudaMemsetAsync(d_counts, 0, sizeof(uint32_t) * n_batch, st));
-    static const bool force_v0 = getenv("FDAS_CORRELATE_V0") != nullptr;
+    const bool force_v0 = getenv("FDAS_CORRELATE_V0") != nullptr;
     if (p->L == 2048 && !force_v0) {
-        static const int env_chunks = getenv("FDAS_T_CHUNKS") ? atoi(getenv("FDAS_T_CHUNKS")) : 0;
+        const int env_chunks = getenv("FDAS_T_CHUNKS") ? atoi(getenv("FDAS_T_CHUNKS")) : 0;
         int n_chunk = env_chunks > 0 ? env_chunks : (p->n_t + 28) / 29;      // ~29 templates per CTA: short tail
         int t_chunk = (p->n_t + n_chunk - 1) / n_chunk;
         n_chunk = (p->n_t + t_chunk - 1) / t_chunk;
@@ -404,8 +404,9 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
         if (d_plane && d_cands) K<true, true, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS); \
         else if (d_plane) K<true, false, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);      \
         else K<false, true, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS)
-        static const bool use_v1 = getenv("FDAS_CORRELATE_V1") != nullptr;
-        static const bool scalar = getenv("FDAS_CORRELATE_SCALAR") != nullptr;     // v2 with scalar FFMA butterflies
+        // tuning switches, read at every call (a few hundred ns) so that one process can time the variants
+        const bool use_v1 = getenv("FDAS_CORRELATE_V1") != nullptr;
+        const bool scalar = getenv("FDAS_CORRELATE_SCALAR") != nullptr;     // v2 with scalar FFMA butterflies
         const bool keep7 = p->step == 7 * 256;                    // m = 256: full segments keep t3 < 7 exactly
 #define FDAS_V2_LAUNCH(NS)                                                                                        \
         if (keep7 && !scalar) { FDAS_V1_LAUNCH(k_correlate_2048_v2, NS, 7, true); }                               \

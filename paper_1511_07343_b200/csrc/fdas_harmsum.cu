@@ -274,11 +274,11 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     for (int i = 0; i < 5; i++) thr.t[i] = i < n_stage ? h_thr[i] : 3.0e38f;
     FDAS_CUDA(cudaMemsetAsync(d_count, 0, sizeof(uint32_t), st));
     int n_cols = (int)p->n_cols;
-    static const int variant = getenv("FDAS_HS_VARIANT") ? atoi(getenv("FDAS_HS_VARIANT")) : 0;
+    const int variant = getenv("FDAS_HS_VARIANT") ? atoi(getenv("FDAS_HS_VARIANT")) : 0;
     // sectors of the tile order (see k_harmsum): 16 by default, thin enough for the reuse distance to fit in
     // L2, thick enough (~10 rows at the far end) for L1 to keep serving the row-direction reuse inside a stream
-    static const int env_sectors = getenv("FDAS_HS_SECTORS") ? atoi(getenv("FDAS_HS_SECTORS")) : 16;
-    static const int env_rows = getenv("FDAS_HS_ROWS") ? atoi(getenv("FDAS_HS_ROWS")) : 0;
+    const int env_sectors = getenv("FDAS_HS_SECTORS") ? atoi(getenv("FDAS_HS_SECTORS")) : 16;
+    const int env_rows = getenv("FDAS_HS_ROWS") ? atoi(getenv("FDAS_HS_ROWS")) : 0;
     int n_sec = env_sectors < 1 ? 1 : env_sectors;
     if (n_sec > HS_MAX_SECTORS) n_sec = HS_MAX_SECTORS;
     int rows = env_rows > 0 ? env_rows : (n_sec == 1 ? HS_ROWS_PER_PASS : 1);      // warps per CTA; each takes a run of consecutive rows (all rows of a sector tile: longest runs)

@@ -188,6 +188,39 @@ def test_time_domain_trial_end_to_end(emu):
     plan.close()
 
 
+def test_correlate_variants_agree(emu):
+    """The kernel variants kept for tuning (FDAS_* switches, read at every call): the packed f32x2 butterflies
+    give the scalar ones' plane bit for bit; the previous kernel (v1) and the generic shared-memory kernel
+    (v0) agree to rounding; the harmonic sum does not depend on its sector count."""
+    cfg = synth.small_config(1 << 13, 12.0, 2.0, 256, 2048, n_sig=2, index=7, amp=0.2)
+    plan = emu.Plan(cfg.n_samples, cfg.z_max, cfg.dz, cfg.width, cfg.seg_len, quad_points=2048)
+    d_S, _ = plan.spectrum(cfg.series())
+    planes = {}
+    for name, env in (("packed", {}), ("scalar", {"FDAS_CORRELATE_SCALAR": "1"}), ("v1", {"FDAS_CORRELATE_V1": "1"}),
+                      ("v0", {"FDAS_CORRELATE_V0": "1"})):
+        os.environ.update(env)
+        try:
+            d_P = plan.correlate(d_S, True)[0]                        # keep the buffer alive while it is copied
+            planes[name] = d_P.np().copy()
+        finally:
+            for k in env:
+                os.environ.pop(k)
+    assert np.array_equal(planes["packed"], planes["scalar"])
+    for other in ("v1", "v0"):
+        assert np.max(np.abs(planes[other] - planes["packed"])) <= 2e-5 * planes["packed"].max()
+    thr = oracle.thresholds(16, 1e-3)
+    lists = []
+    for sectors in ("1", "16", "7"):
+        os.environ["FDAS_HS_SECTORS"] = sectors
+        try:
+            c, n = plan.harmsum(E.to_dev(planes["packed"][0]), 16, thr, 1 << 16)
+        finally:
+            os.environ.pop("FDAS_HS_SECTORS")
+        lists.append(sorted((int(r["nharm"]), int(r["zi"]), int(r["col"]), float(r["power"])) for r in c))
+    assert lists[0] == lists[1] == lists[2] and len(lists[0]) > 0
+    plan.close()
+
+
 def test_fused_batch(emu):
     small = synth.small_config(1 << 13, 8.0, 2.0, 64, 2048, n_dm=5, n_sig=1, index=33, amp=0.3)
     xs = np.stack([small.series(d) for d in range(5)])

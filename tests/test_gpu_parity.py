@@ -341,6 +341,41 @@ def test_time_domain_trial_end_to_end(fdas):
     assert float(d_Pf.max()) == pytest.approx(float(d_P.max()), rel=0.15)
 
 
+def test_kernel_variants_agree(fdas):
+    """The variants kept for tuning (FDAS_* switches, read at every call): packed f32x2 butterflies give the
+    scalar ones' plane bit for bit, v1 agrees to rounding, the harmonic sum does not depend on its sector count."""
+    import os
+    cfg = synth.small_config(1 << 16, 40.0, 2.0, 256, 2048, n_sig=2, index=7, amp=0.1)
+    plan = make_plan(fdas, cfg)
+    d_S, _ = plan.spectrum(torch.from_numpy(cfg.series()).cuda().view(1, -1))
+    planes = {}
+    for name, env in (("packed", {}), ("scalar", {"FDAS_CORRELATE_SCALAR": "1"}), ("v1", {"FDAS_CORRELATE_V1": "1"})):
+        os.environ.update(env)
+        try:
+            d_P = plan.empty_plane(1)
+            plan.correlate(d_S, d_P)
+            planes[name] = d_P[0].cpu().numpy()
+        finally:
+            for k in env:
+                os.environ.pop(k)
+    assert np.array_equal(planes["packed"], planes["scalar"])
+    assert np.max(np.abs(planes["v1"] - planes["packed"])) <= 2e-5 * planes["packed"].max()
+    thr = oracle.thresholds(16, 1e-4)
+    d_P = torch.from_numpy(planes["packed"]).cuda()
+    lists = []
+    for env in ({"FDAS_HS_SECTORS": "1"}, {}, {"FDAS_HS_SECTORS": "32"}, {"FDAS_HS_VARIANT": "1"}):
+        os.environ.update(env)
+        try:
+            cands = plan.empty_cands(1 << 18)
+            plan.harmsum(d_P, 16, thr, cands, 1 << 18)
+            c = fdas.cands_to_numpy(*cands)
+        finally:
+            for k in env:
+                os.environ.pop(k)
+        lists.append(sorted((int(r["nharm"]), int(r["zi"]), int(r["col"]), float(r["power"])) for r in c))
+    assert all(l == lists[0] for l in lists) and len(lists[0]) > 0
+
+
 def test_maximum_series_length(fdas):
     """The largest series the plan accepts (2^25 samples; 2^24 columns per row): index arithmetic at its
     limits (k h, plane indices, twiddle phases), 3 templates to keep the oracle's share small."""
