@@ -205,7 +205,7 @@ def run_ab(args):
         out["correlate_ms"][name] = timed(corr, env)
     corr()
     for name, env in (("S16", {}), ("S1", {"FDAS_HS_SECTORS": "1"}), ("S8", {"FDAS_HS_SECTORS": "8"}),
-                      ("S32", {"FDAS_HS_SECTORS": "32"}), ("S16_rows2", {"FDAS_HS_ROWS": "2"}),
+                      ("S32", {"FDAS_HS_SECTORS": "32"}), ("S16_1warp", {"FDAS_HS_ROWS": "1"}), ("S16_8warps", {"FDAS_HS_ROWS": "8"}),
                       ("S16_128col", {"FDAS_HS_VARIANT": "1"}), ("S32_128col", {"FDAS_HS_VARIANT": "1", "FDAS_HS_SECTORS": "32"})):
         out["harmsum_ms"][name] = timed(hs, env)
         out.setdefault("harmsum_candidates", {})[name] = int(cands[1][0])

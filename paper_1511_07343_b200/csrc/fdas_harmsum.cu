@@ -38,7 +38,8 @@ __device__ __noinline__ void push_cand_hs(fdas_cand* list, uint32_t* count, uint
 template <int NST, int HS_CPT, bool CHECK>
 __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fdas_cand* __restrict__ cands,
                                              uint32_t* __restrict__ count, uint32_t cap, const HarmThr& thr,
-                                             int n_cols, int n_z, int bin0, int tile, int zi_lo, int zi_hi)
+                                             int n_cols, int n_z, int bin0, int tile, int zi_lo, int zi_hi,
+                                             int row_part, int n_row_parts)
 {
     constexpr int HS_COLS = 32 * HS_CPT;
     constexpr int HMAX = 1 << (NST - 1);
@@ -46,8 +47,8 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
     const int col0 = tile * HS_COLS + lane;
     const int zc = (n_z - 1) / 2;
     const int k = bin0 + col0;
-    const int rpw = (zi_hi - zi_lo + (int)blockDim.y - 1) / (int)blockDim.y;
-    const int r_begin = zi_lo + (int)threadIdx.y * rpw, r_end = min(zi_hi, r_begin + rpw);
+    const int rpw = (zi_hi - zi_lo + n_row_parts - 1) / n_row_parts;
+    const int r_begin = zi_lo + row_part * rpw, r_end = min(zi_hi, r_begin + rpw);
     if (r_begin >= r_end) return;                                      // the whole warp
 
     // this lane's slot for the ballot (lanes 0 and >= HMAX never report a move)
@@ -164,7 +165,9 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
 constexpr int HS_MAX_SECTORS = 64;
 struct HarmSectors {
     int n_sec;
-    int first_item[HS_MAX_SECTORS + 1];      // sector s owns items [first_item[s], first_item[s+1]): its column tiles 0, 1, ...
+    int col_warps;                           // > 1: the warps of a CTA take ADJACENT column tiles (all rows each) and share
+                                             // the L1 lines at the seams; 1: they split the rows of one tile (plain order)
+    int first_item[HS_MAX_SECTORS + 1];      // sector s owns items [first_item[s], first_item[s+1]): its groups of col_warps tiles
 };
 
 __host__ __device__ inline double sector_boundary(int j, int S, double kc, double K, double zhalf)
@@ -185,30 +188,36 @@ k_harmsum(const float* __restrict__ plane, fdas_cand* __restrict__ cands, uint32
     const int zc = (n_z - 1) / 2;
     const double K = (double)(bin0 + n_cols - 1), zhalf = 0.5 * (double)n_z;
     const int n_items = sec.first_item[sec.n_sec];
+    const int n_tiles = (n_cols + HS_COLS - 1) / HS_COLS;
     int s = 0;
 #pragma unroll 1
     for (int item = blockIdx.x; item < n_items; item += gridDim.x) {                // everything here is CTA-uniform
         while (item >= sec.first_item[s + 1]) s++;
-        const int tile = item - sec.first_item[s];
+        const int group = item - sec.first_item[s];
+        const int tile_last = min(n_tiles, (group + 1) * sec.col_warps) - 1;
         int zi_lo = 0, zi_hi = n_z;
-        if (sec.n_sec > 1) {                 // rows of this sector, taken at the last bin of the tile
-            const double kc = (double)bin0 + (double)min(n_cols, (tile + 1) * HS_COLS) - 1.0;
+        if (sec.n_sec > 1) {                 // rows of this sector, taken at the last bin of the group of tiles
+            const double kc = (double)bin0 + (double)min(n_cols, (tile_last + 1) * HS_COLS) - 1.0;
             zi_lo = max(0, min(n_z, (int)ceil(sector_boundary(s, sec.n_sec, kc, K, zhalf)) + zc));
             zi_hi = max(0, min(n_z, (int)ceil(sector_boundary(s + 1, sec.n_sec, kc, K, zhalf)) + zc));
             if (zi_lo >= zi_hi) continue;
         }
+        const int tile = sec.col_warps > 1 ? group * sec.col_warps + (int)threadIdx.y : group;       // warp-uniform
+        if (tile >= n_tiles) continue;
+        const int row_part = sec.col_warps > 1 ? 0 : (int)threadIdx.y, n_row_parts = sec.col_warps > 1 ? 1 : (int)blockDim.y;
         const bool edge = tile == 0 || tile * HS_COLS + HS_COLS > n_cols;
-        if (edge) harmsum_tile<NST, HS_CPT, true>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi);
-        else harmsum_tile<NST, HS_CPT, false>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi);
+        if (edge) harmsum_tile<NST, HS_CPT, true>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi, row_part, n_row_parts);
+        else harmsum_tile<NST, HS_CPT, false>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi, row_part, n_row_parts);
     }
 }
 
 // Sector -> item ranges.  A sector whose two boundary rays both leave through the top/bottom edge is empty
 // beyond the column where the shallower one leaves; only the tiles before that become items.
-static HarmSectors make_sectors(int n_sec, int n_cols, int bin0, int cols_per_tile)
+static HarmSectors make_sectors(int n_sec, int col_warps, int n_cols, int bin0, int cols_per_tile)
 {
     HarmSectors hs;
     hs.n_sec = n_sec;
+    hs.col_warps = col_warps;
     const int n_tiles = (n_cols + cols_per_tile - 1) / cols_per_tile;
     const double K = (double)(bin0 + n_cols - 1);
     hs.first_item[0] = 0;
@@ -218,11 +227,11 @@ static HarmSectors make_sectors(int n_sec, int n_cols, int bin0, int cols_per_ti
             const double ua = -2.0 + 4.0 * s / n_sec, ub = -2.0 + 4.0 * (s + 1) / n_sec;
             const double umin = fabs(ua) < fabs(ub) ? fabs(ua) : fabs(ub);
             if (ua * ub > 0.0 && umin > 1.0) {
-                const long long t = (long long)(K * (2.0 - umin) / cols_per_tile) + 2;
+                const long long t = ((long long)(K * (2.0 - umin) / (cols_per_tile * col_warps)) + 2) * col_warps;
                 if (t < nt) nt = (int)t;
             }
         }
-        hs.first_item[s + 1] = hs.first_item[s] + nt;
+        hs.first_item[s + 1] = hs.first_item[s] + (nt + col_warps - 1) / col_warps;
     }
     return hs;
 }
@@ -281,13 +290,14 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     const int env_rows = getenv("FDAS_HS_ROWS") ? atoi(getenv("FDAS_HS_ROWS")) : 0;
     int n_sec = env_sectors < 1 ? 1 : env_sectors;
     if (n_sec > HS_MAX_SECTORS) n_sec = HS_MAX_SECTORS;
-    int rows = env_rows > 0 ? env_rows : (n_sec == 1 ? HS_ROWS_PER_PASS : 1);      // warps per CTA; each takes a run of consecutive rows (all rows of a sector tile: longest runs)
+    int rows = env_rows > 0 ? env_rows : (n_sec == 1 ? HS_ROWS_PER_PASS : 4);      // warps per CTA: with sectors, 4 adjacent column tiles (all rows of the
+                                                                                    // sector each: longest carried runs); plain order: 8 row parts of one tile
     if (rows > HS_ROWS_PER_PASS) rows = HS_ROWS_PER_PASS;
     dim3 block(32, rows);
     HarmSectors sec;
 #define FDAS_HS_LAUNCH(NST, CPT, MINB)                                                              \
     do {                                                                                            \
-        sec = make_sectors(n_sec, n_cols, p->bin0, 32 * CPT);                                       \
+        sec = make_sectors(n_sec, n_sec == 1 ? 1 : rows, n_cols, p->bin0, 32 * CPT);                                       \
         int n_cta = resident_ctas(k_harmsum<NST, CPT, MINB>, 32 * rows);                            \
         if (n_cta > sec.first_item[n_sec]) n_cta = sec.first_item[n_sec];                           \
         k_harmsum<NST, CPT, MINB><<<dim3(n_cta), block, 0, st>>>(                                   \
