@@ -170,8 +170,11 @@ unsigned emu_ballot(int pred)
     return r;
 }
 
-static void run_block(Worker* w, dim3 block, bool rev)
+static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward, 1 reversed, >= 2 pseudo-random (seed)
 {
+    const bool rev = order == 1;
+    uint64_t rng = 0x9E3779B97F4A7C15ull * (uint64_t)(order + 1) + blockIdx.x * 0x632BE59BD9B4E019ull + blockIdx.y * 977 + blockIdx.z;
+    std::vector<int> perm;
     const int nt = block.x * block.y * block.z;
     if ((int)w->fibers.size() < nt) {
         size_t old = w->fibers.size();
@@ -189,8 +192,16 @@ static void run_block(Worker* w, dim3 block, bool rev)
     int done = 0;
     while (done < nt) {
         bool progress = false;
+        if (order >= 2) {                        // a fresh random order of the threads for every scheduling round
+            perm.resize(nt);
+            for (int q = 0; q < nt; q++) perm[q] = q;
+            for (int q = nt - 1; q > 0; q--) {
+                rng ^= rng << 13; rng ^= rng >> 7; rng ^= rng << 17;
+                std::swap(perm[q], perm[(int)(rng % (uint64_t)(q + 1))]);
+            }
+        }
         for (int q = 0; q < nt; q++) {
-            int i = rev ? nt - 1 - q : q;
+            int i = order >= 2 ? perm[q] : (rev ? nt - 1 - q : q);
             Fiber& f = w->fibers[i];
             if (f.state != ST_RUN) continue;
             w->cur = i;
@@ -244,7 +255,8 @@ void emu_launch(dim3 grid, dim3 block, size_t smem, const char* name, const std:
     }
     const long nblocks = (long)grid.x * grid.y * grid.z;
     std::atomic<long> next{0};
-    const bool rev = getenv("EMU_ORDER") && !strcmp(getenv("EMU_ORDER"), "rev");
+    const char* eo = getenv("EMU_ORDER");
+    const int rev = !eo ? 0 : !strcmp(eo, "rev") ? 1 : !strncmp(eo, "rand", 4) ? 2 + atoi(eo + 4) : 0;
     int nthr = getenv("EMU_THREADS") ? atoi(getenv("EMU_THREADS")) : (int)std::thread::hardware_concurrency();
     if (nthr > nblocks) nthr = (int)nblocks;
     if (nthr < 1) nthr = 1;

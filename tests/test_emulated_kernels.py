@@ -24,9 +24,11 @@ from emu import harness as E  # noqa: E402
 fdas = E.fdas
 
 
-@pytest.fixture(params=[("end", "fwd"), ("start", "rev")], ids=["guard-after", "guard-before-reversed"])
+@pytest.fixture(params=[("end", "fwd"), ("start", "rev"), ("end", "rand7")],
+                ids=["guard-after", "guard-before-reversed", "guard-after-random-order"])
 def emu(request):
-    """Buffer placement against the trailing / leading guard page; thread order within a CTA forward / reversed."""
+    """Buffer placement against the trailing / leading guard page; thread order within a CTA forward / reversed /
+    pseudo-random."""
     os.environ["EMU_ALIGN"], os.environ["EMU_ORDER"] = request.param
     yield E
     os.environ.pop("EMU_ALIGN"), os.environ.pop("EMU_ORDER")
