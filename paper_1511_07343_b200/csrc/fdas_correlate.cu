@@ -281,7 +281,7 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
                 long long c = (long long)c0 - m / 2 + p + 256 * n3;
                 u[bitrev(n3, 3)] = (c >= 0 && c < n_bins) ? S[c] : make_float2(0.f, 0.f);
             }
-            dit_const<8, -1>(u);
+            dit_const<8, -1, PK>(u);
 #pragma unroll
             for (int k3 = 0; k3 < 8; k3++) {
                 float2 val = k3 ? cmul(u[k3], twiddle(k3 * p, L, -1.0f)) : u[0];
@@ -292,7 +292,7 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
         float2 v[16];
 #pragma unroll
         for (int n2 = 0; n2 < 16; n2++) v[bitrev(n2, 4)] = buf[lo + 16 * n2 + V2_PITCH3 * k3A];
-        dit_const<16, -1>(v);
+        dit_const<16, -1, PK>(v);
 #pragma unroll
         for (int k2 = 1; k2 < 16; k2++) v[k2] = cmul(v[k2], twiddle(k2 * lo, 256, -1.0f));
         __syncwarp();
@@ -301,7 +301,7 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
         __syncwarp();
 #pragma unroll
         for (int n1 = 0; n1 < 16; n1++) v[bitrev(n1, 4)] = buf[lo + 18 * n1 + V2_PITCH3 * k3A];
-        dit_const<16, -1>(v);
+        dit_const<16, -1, PK>(v);
 #pragma unroll
         for (int k1 = 0; k1 < 16; k1++) X[k1] = v[k1];
         __syncthreads();

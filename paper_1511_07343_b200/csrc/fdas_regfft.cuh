@@ -127,13 +127,13 @@ __device__ __forceinline__ void dit_const_stage(float2* v)
 }
 
 // DIT on R points (8 or 16), no inter-pass twiddle (w = 1): constants only.
-template <int R, int SIGN>
+template <int R, int SIGN, bool PK = false>
 __device__ __forceinline__ void dit_const(float2* v)
 {
-    dit_const_stage<R, SIGN, 1>(v);
-    dit_const_stage<R, SIGN, 2>(v);
-    dit_const_stage<R, SIGN, 3>(v);
-    if constexpr (R >= 16) dit_const_stage<R, SIGN, 4>(v);
+    dit_const_stage<R, SIGN, 1, PK>(v);
+    dit_const_stage<R, SIGN, 2, PK>(v);
+    dit_const_stage<R, SIGN, 3, PK>(v);
+    if constexpr (R >= 16) dit_const_stage<R, SIGN, 4, PK>(v);
 }
 
 // Template multiply folded into the first (span 2) stage of the 16-point inverse DIT:
