@@ -70,10 +70,10 @@ __device__ __forceinline__ void stockham_pass(const float2* __restrict__ in, flo
             // w4 = w2 w2, w5 = w4 w1, w6 = w3 w3, w7 = w4 w3): a few 1e-8 of extra error, 6 fewer sincospif
             float2 w[R];
             w[1] = twiddle(k, p * R, sign);
-            if (R > 2) { w[2] = cmul(w[1], w[1]); w[3] = cmul(w[2], w[1]); }
-            if (R > 4) { w[4] = cmul(w[2], w[2]); w[5] = cmul(w[4], w[1]); w[6] = cmul(w[3], w[3]); w[7] = cmul(w[4], w[3]); }
+            if (R > 2) { w[2] = cmul_pk(w[1], w[1]); w[3] = cmul_pk(w[2], w[1]); }
+            if (R > 4) { w[4] = cmul_pk(w[2], w[2]); w[5] = cmul_pk(w[4], w[1]); w[6] = cmul_pk(w[3], w[3]); w[7] = cmul_pk(w[4], w[3]); }
 #pragma unroll
-            for (int j = 1; j < R; j++) u[j] = cmul(u[j], w[j]);
+            for (int j = 1; j < R; j++) u[j] = cmul_pk(u[j], w[j]);
         }
         dftR<R>(u, sign);
         int j0 = (i - k) * R + k;

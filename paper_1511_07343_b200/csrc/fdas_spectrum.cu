@@ -42,7 +42,7 @@ k_spec_pass1(const float* __restrict__ series, float2* __restrict__ inter, doubl
         int k1 = idx / C, cc = idx - k1 * C;
         int n2 = n2_0 + cc;
         int ph = (int)(((long long)n2 * k1) & (M - 1));
-        float2 v = cmul(r[cc * pitch + k1], twiddle(ph, M, -1.0f));
+        float2 v = cmul_pk(r[cc * pitch + k1], twiddle(ph, M, -1.0f));
         inter[(size_t)bt * M + (size_t)k1 * R2 + n2] = v;
     }
     // block reduction of the three sums (fixed tree)
@@ -120,7 +120,7 @@ k_spec_pass2(const float2* __restrict__ inter, const double* __restrict__ part, 
         float2 dd = make_float2(0.5f * (zk.x - zp.x), 0.5f * (zk.y + zp.y));     // (Z_k - conj Z_{M-k})/2
         float2 o = make_float2(dd.y, -dd.x);                                      // * (-i)
         float2 w = twiddle(k, 2 * M, -1.0f);
-        float2 f = cadd(e, cmul(o, w));
+        float2 f = cadd(e, cmul_pk(o, w));
         out[k - 1] = make_float2(f.x * sc, f.y * sc);
     }
 }
