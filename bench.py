@@ -70,6 +70,20 @@ class ClockSampler:
                 "reasons": reasons, "samples": len(sm)}
 
 
+def host_description():
+    """CPU model and the oracle's compiler flags, for the cpu_baseline record."""
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except OSError:
+        pass
+    import oracle
+    return {"cpu_model": model, "nproc": os.cpu_count(), "oracle_cflags": " ".join(getattr(oracle, "CFLAGS", []))}
+
+
 def oracle_sample(cfg, x, frac_log2=4):
     """Time the oracle, as it stands, on a bounded sample of one DM trial: the full O1 spectrum, then
     O7 overlap-save correlation + O6 harmonic sum on the first n_bins/2^frac_log2 bins; extrapolate."""
@@ -116,7 +130,7 @@ def run_reference(args):
         "config": {"workload": "BASELINE.json configs[2] (SKA beam, single DM) + configs[4] harmonic sum",
                    "n_samples": cfg.n_samples, "n_z": cfg.n_z, "width": cfg.width, "segment_len": cfg.seg_len},
         "cpu_baseline": {"value": val, "unit": UNIT, "cores": detail["cores"], "kind": "oracle",
-                         "sample": detail["sample"]},
+                         "sample": detail["sample"], **host_description()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
     }))
 
@@ -422,7 +436,7 @@ def run_ours(args):
         t_dm, d = oracle_sample(cfg, base, frac_log2=4)
         out["cpu_baseline"] = {"value": 1.0 / t_dm, "unit": UNIT, "cores": d["cores"], "kind": "oracle",
                                "sample": d["sample"], "spectrum_s": d["spectrum_s"],
-                               "correlate_fft_s": d["correlate_fft_s"], "harmsum_s": d["harmsum_s"]}
+                               "correlate_fft_s": d["correlate_fft_s"], "harmsum_s": d["harmsum_s"], **host_description()}
     print(json.dumps(out))
     if world > 1:
         dist.destroy_process_group()
