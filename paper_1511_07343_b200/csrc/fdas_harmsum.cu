@@ -85,6 +85,10 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
         }
     }
     static_assert(HS_CPT % 2 == 0, "cells are summed in pairs (packed f32x2 adds)");
+    // the row stride in a register of its own: otherwise every predicated index update re-reads it from the
+    // constant bank (an LDC per stream and row)
+    // (ptxas re-materialises a plain copy of a kernel parameter; gridDim.y is 1, which it cannot know)
+    const int stride = n_cols + (int)gridDim.y - 1;
     float2 v[HS_CPT / 2][HMAX];                                       // .x, .y = cells 2jj, 2jj+1 of the lane
 #define HS_V(j, i) (((j) & 1) ? v[(j) >> 1][i].y : v[(j) >> 1][i].x)
     for (int zi = r_begin; zi < r_end; zi++) {
@@ -97,7 +101,7 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
             const float* src = plane + idx[0];
 #pragma unroll
             for (int j = 0; j < HS_CPT; j++) HS_V(j, 0) = (!CHECK || (okmask >> j & 1)) ? __ldcs(src + 32 * j) : 0.0f;
-            idx[0] += n_cols;
+            idx[0] += stride;
         }
 #pragma unroll
         for (int st = 1; st < NST; st++) {
@@ -106,7 +110,7 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
             for (int h = 1; h < H; h += 2) {
                 const int slot = (H >> 1) + (h >> 1);
                 if (moved & (1u << slot)) {                            // warp-uniform
-                    idx[slot] += n_cols;
+                    idx[slot] += stride;
                     const float* src = plane + idx[slot];
                     const int dk = (32 * h) >> st;                     // exact: 32 h / H
 #pragma unroll
