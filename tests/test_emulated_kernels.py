@@ -255,3 +255,36 @@ def test_search_host(emu):
     h_c, h_n = fdas.fdas_search_host(plan.handle, xs, 4, fdas.thresholds(4, 1e-3), 1 << 14)
     assert h_n[0] == h_n[2] and cset(h_c[0, :h_n[0]]) == cset(h_c[2, :h_n[2]])
     plan.close()
+
+
+def test_the_emulator_catches_out_of_bounds_and_misaligned_accesses():
+    """The harness itself: a plane buffer that is too short, or a misaligned one, must stop the run (guard page:
+    exit code 99 with the kernel named; alignment sanitizer: abort) -- otherwise the tests above prove nothing."""
+    import subprocess
+    prog = r'''
+import sys, numpy as np
+sys.path.insert(0, %r)
+from emu import harness as E
+plan = E.Plan(1 << 12, 4.0, 2.0, 16, 256, quad_points=64)
+n = plan.info.n_z * plan.info.n_cols
+mode = sys.argv[1]
+if mode == "short":
+    buf = E.DevBuf(n - 64, np.float32); buf.np()[...] = 1.0
+    class P:                                            # the kernel reads n cells from a buffer of n - 64
+        def data_ptr(self): return buf.ptr
+    plan.candidates(P(), 0.5, 16)
+else:
+    d_S, _ = plan.spectrum(np.zeros(1 << 12, np.float32))
+    buf = E.DevBuf(n + 4, np.float32)
+    class P:
+        def data_ptr(self): return buf.ptr + 4          # 4-byte offset: the boundary must refuse it
+    try:
+        E.fdas.fdas_correlate(plan.handle, d_S, 1, P(), 0.0, None, None, 0)
+    except E.fdas.FdasError as e:
+        sys.exit(0 if e.code == E.fdas.FDAS_E_INVALID else 3)
+    sys.exit(4)
+''' % os.path.dirname(os.path.abspath(__file__))
+    short = subprocess.run([sys.executable, "-c", prog, "short"], capture_output=True, text=True, timeout=300)
+    assert short.returncode == 99 and "illegal access" in short.stderr and "k_candidates" in short.stderr, short.stderr[-500:]
+    mis = subprocess.run([sys.executable, "-c", prog, "misaligned"], capture_output=True, text=True, timeout=300)
+    assert mis.returncode == 0, mis.stderr[-500:]
