@@ -31,7 +31,7 @@ def workload_flops(info):
     """Algorithmic flops of the fused correlate kernel per DM trial (SURVEY.md §8(d) convention:
     5 L log2 L per complex FFT, 6 per complex multiply, 3 per power)."""
     L, m, n_t, n_bins = info.seg_len, info.width, info.n_templates, info.n_bins
-    n_seg = math.ceil(n_bins / (L - m + 1))
+    n_seg = math.ceil(n_bins / (L - m + 1))       # the minimum segmentation at this L, m (the library's step L - m gives one more)
     return n_seg * (5 * L * math.log2(L) * (1 + n_t) + 6 * L * n_t) + 3 * n_t * n_bins
 
 
@@ -118,7 +118,7 @@ def run_reference(args):
     x = cfg.series()
     times, detail = [], None
     for i in range(args.warmup + args.steps):
-        t_dm, detail = oracle_sample(cfg, x, frac_log2=5)
+        t_dm, detail = oracle_sample(cfg, x, frac_log2=4)
         if i >= args.warmup:
             times.append(t_dm)
     t = sum(times) / len(times)
@@ -176,9 +176,9 @@ def run_sweep(args):
 
 
 def run_ab(args):
-    """--ab: time the kernel variants kept for tuning, in one process (the library reads its FDAS_* switches
-    at every call): fused correlate v1 / v2 scalar / v2 packed, harmonic sum for several sector counts and
-    the 128-column variant.  One JSON line; nothing here is a bench value."""
+    """--ab: time the tuning keys (FDAS_OPT_TUNE_*) in one process: fused correlate scalar / packed and its
+    template chunking, harmonic sum for several sector counts and tile shapes.  One JSON line; nothing here
+    is a bench value."""
     import torch
     from paper_1511_07343_b200 import build as fbuild, fdas, synth
     torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", "0")))
@@ -193,11 +193,9 @@ def run_ab(args):
     thr = fdas.thresholds(16)
     stream = torch.cuda.current_stream()
 
-    def timed(fn, env):
-        keys = [k for k in os.environ if k.startswith("FDAS_")]
-        for k in keys:
-            del os.environ[k]
-        os.environ.update(env)
+    def timed(fn, opts):
+        for k, v in opts.items():
+            fdas.fdas_plan_set_option(plan.handle, k, v)
         for _ in range(3):
             fn()
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -207,21 +205,25 @@ def run_ab(args):
             fn()
         e1.record(stream)
         torch.cuda.synchronize()
-        for k in env:
-            del os.environ[k]
+        for k in opts:
+            fdas.fdas_plan_set_option(plan.handle, k, 0)
         return e0.elapsed_time(e1) / args.steps
 
     corr = lambda: fdas.fdas_correlate(plan.handle, d_spec, 1, d_plane, 0.0, None, None, 0)
     hs = lambda: fdas.fdas_harmsum(plan.handle, d_plane[0], 16, thr, cands[0], cands[1], cap)
     out = {"correlate_ms": {}, "harmsum_ms": {}, "steps": args.steps}
-    for name, env in (("v2_packed", {}), ("v2_scalar", {"FDAS_CORRELATE_SCALAR": "1"}), ("v1", {"FDAS_CORRELATE_V1": "1"}),
-                      ("v2_packed_4chunks", {"FDAS_T_CHUNKS": "4"}), ("v2_packed_2chunks", {"FDAS_T_CHUNKS": "2"})):
-        out["correlate_ms"][name] = timed(corr, env)
+    F = fdas
+    for name, opts in (("packed", {}), ("scalar", {F.FDAS_OPT_TUNE_SCALAR: 1}),
+                       ("packed_1chunk", {F.FDAS_OPT_TUNE_T_CHUNKS: 1}), ("packed_2chunks", {F.FDAS_OPT_TUNE_T_CHUNKS: 2}),
+                       ("packed_4chunks", {F.FDAS_OPT_TUNE_T_CHUNKS: 4}), ("packed_6chunks", {F.FDAS_OPT_TUNE_T_CHUNKS: 6})):
+        out["correlate_ms"][name] = timed(corr, opts)
     corr()
-    for name, env in (("S16", {}), ("S1", {"FDAS_HS_SECTORS": "1"}), ("S8", {"FDAS_HS_SECTORS": "8"}),
-                      ("S32", {"FDAS_HS_SECTORS": "32"}), ("S16_1warp", {"FDAS_HS_ROWS": "1"}), ("S16_8warps", {"FDAS_HS_ROWS": "8"}),
-                      ("S16_128col", {"FDAS_HS_VARIANT": "1"}), ("S32_128col", {"FDAS_HS_VARIANT": "1", "FDAS_HS_SECTORS": "32"})):
-        out["harmsum_ms"][name] = timed(hs, env)
+    for name, opts in (("S16", {}), ("S1", {F.FDAS_OPT_TUNE_HS_SECTORS: 1}), ("S8", {F.FDAS_OPT_TUNE_HS_SECTORS: 8}),
+                       ("S32", {F.FDAS_OPT_TUNE_HS_SECTORS: 32}), ("S64", {F.FDAS_OPT_TUNE_HS_SECTORS: 64}),
+                       ("S16_1warp", {F.FDAS_OPT_TUNE_HS_ROWS: 1}),
+                       ("S16_8warps", {F.FDAS_OPT_TUNE_HS_ROWS: 8}), ("S16_128col", {F.FDAS_OPT_TUNE_HS_VARIANT: 1}),
+                       ("S32_128col", {F.FDAS_OPT_TUNE_HS_VARIANT: 1, F.FDAS_OPT_TUNE_HS_SECTORS: 32})):
+        out["harmsum_ms"][name] = timed(hs, opts)
         out.setdefault("harmsum_candidates", {})[name] = int(cands[1][0])
     print(json.dumps(out))
 

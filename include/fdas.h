@@ -50,6 +50,13 @@ extern "C" {
 #define FDAS_OPT_INTERBIN     1  /* 0/1: add the half-bin template set (BJ:configs[1]); default 0 */
 #define FDAS_OPT_MAX_BATCH    2  /* largest n_batch the calls will see (sizes workspace_bytes); default 1 */
 #define FDAS_OPT_QUAD_POINTS  3  /* quadrature points of the template generator; default 32768 */
+/* Tuning keys: launch geometry / instruction selection only, results do not depend on them; may be set at
+ * any time; 0 = the default.  Kept for A/B timing (bench.py --ab). */
+#define FDAS_OPT_TUNE_SCALAR     101  /* 1: scalar FFMA butterflies in the L = 2048 segment kernel (default: packed FFMA2) */
+#define FDAS_OPT_TUNE_T_CHUNKS   102  /* template chunks per segment in the L = 2048 segment kernel (default ceil(n_t/29)) */
+#define FDAS_OPT_TUNE_HS_SECTORS 103  /* angular sectors of the harmonic-sum tile order, 1..64 (default 16) */
+#define FDAS_OPT_TUNE_HS_ROWS    104  /* warps per CTA of the harmonic-sum kernel, 1..8 (default 4) */
+#define FDAS_OPT_TUNE_HS_VARIANT 105  /* 1: 128-column harmonic-sum tiles (default 64) */
 
 typedef struct fdas_plan fdas_plan;
 
@@ -78,13 +85,14 @@ int fdas_set_device(int32_t device);
  * z = -z_max .. z_max step dz ("multiple templates"; z = fdot*T^2 = bins
  * drifted over the span), each an FIR of `template_width` taps, by
  * overlap-save with segments of `segment_len` bins (PAPER.md:49 step 3).
- * FDAS_E_INVALID unless: n_samples a power of two with 2*segment_len <= n_samples <= 2^26;
+ * FDAS_E_INVALID unless: n_samples a power of two with 2*segment_len <= n_samples <= 2^25 (the fp32 twiddle
+ * arguments k/N are exact up to there);
  * segment_len in {256, 512, 1024, 2048, 4096}; template_width even, >= 2 and
  * <= segment_len/2; dz > 0, z_max >= 0 and z_max/dz an integer; n_z <= 32767. */
 int fdas_plan_create(fdas_plan** out, int64_t n_samples, double z_max, double dz,
                      int32_t template_width, int32_t segment_len);
 
-/* Options must be set before fdas_build_templates (else FDAS_E_STATE). */
+/* Options 1..3 must be set before fdas_build_templates (else FDAS_E_STATE); tuning keys any time. */
 int fdas_plan_set_option(fdas_plan* plan, int32_t key, int64_t value);
 
 int fdas_plan_info(const fdas_plan* plan, fdas_info* out);
@@ -179,12 +187,12 @@ double fdas_threshold(int32_t n_harm, double pfa);
 
 /* Measurement aid: the FP32 fused-multiply-add rate of the current device in
  * TFLOP/s, from a kernel of independent FFMA chains (a <- a*x + y) on every SM, best of 4 timed
- * launches with CUDA events on `stream`; *out_ms (may be NULL) receives that launch's duration, and a
- * NEGATIVE *out_ms on entry selects the same chains written with the packed f32x2 instruction of sm_100
- * (FFMA2, two FMAs per lane and issue slot) so that both rates can be reported.
+ * launches with CUDA events on `stream`; *out_ms (may be NULL) receives that launch's duration.
+ * packed = 1 selects the same chains written with the packed f32x2 instruction of sm_100 (FFMA2, two
+ * FMAs per lane and issue slot) so that both rates can be reported.
  * bench.py reports the fused correlate kernel against this measured peak as well as the nominal one.
  * Synchronises `stream`; allocates and frees 4 bytes of device memory.  Not part of the search path. */
-int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, void* stream);
+int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, int32_t packed, void* stream);
 
 int fdas_plan_destroy(fdas_plan* plan);
 

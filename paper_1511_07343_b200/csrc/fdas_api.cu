@@ -85,6 +85,14 @@ extern "C" int fdas_plan_create(fdas_plan** out, int64_t n_samples, double z_max
 extern "C" int fdas_plan_set_option(fdas_plan* p, int32_t key, int64_t value)
 {
     if (!p) return FDAS_E_INVALID;
+    switch (key) {                        // tuning keys: any time, results do not depend on them
+    case FDAS_OPT_TUNE_SCALAR:     if (value != 0 && value != 1) return FDAS_E_INVALID; p->tune_scalar = (int32_t)value; return FDAS_OK;
+    case FDAS_OPT_TUNE_T_CHUNKS:   if (value < 0 || value > 1024) return FDAS_E_INVALID; p->tune_t_chunks = (int32_t)value; return FDAS_OK;
+    case FDAS_OPT_TUNE_HS_SECTORS: if (value < 0 || value > 64) return FDAS_E_INVALID; p->tune_hs_sectors = (int32_t)value; return FDAS_OK;
+    case FDAS_OPT_TUNE_HS_ROWS:    if (value < 0 || value > 8) return FDAS_E_INVALID; p->tune_hs_rows = (int32_t)value; return FDAS_OK;
+    case FDAS_OPT_TUNE_HS_VARIANT: if (value < 0 || value > 1) return FDAS_E_INVALID; p->tune_hs_variant = (int32_t)value; return FDAS_OK;
+    default: break;
+    }
     if (p->built) return FDAS_E_STATE;
     switch (key) {
     case FDAS_OPT_INTERBIN:
@@ -120,11 +128,10 @@ extern "C" int fdas_build_templates(fdas_plan* p, void* stream)
 {
     if (!p) return FDAS_E_INVALID;
     cudaStream_t st = (cudaStream_t)stream;
-    if (!p->d_taps) {
-        if (cudaMalloc(&p->d_taps, (size_t)p->n_t * p->m * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); return FDAS_E_NOMEM; }
-        if (cudaMalloc(&p->d_W, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); return FDAS_E_NOMEM; }
-        if (cudaMalloc(&p->d_Wr, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { cudaGetLastError(); return FDAS_E_NOMEM; }
-    }
+    if (p->built) return FDAS_OK;                                  // the bank is built once
+    if (!p->d_taps && cudaMalloc(&p->d_taps, (size_t)p->n_t * p->m * sizeof(float2)) != cudaSuccess) { p->d_taps = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
+    if (!p->d_W && cudaMalloc(&p->d_W, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { p->d_W = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
+    if (!p->d_Wr && cudaMalloc(&p->d_Wr, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { p->d_Wr = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
     int rc = fdas_launch_templates(p, st);
     if (rc) return rc;
     FDAS_CUDA(cudaStreamSynchronize(st));
@@ -155,7 +162,7 @@ extern "C" int fdas_correlate(fdas_plan* p, const float* d_spectrum, int32_t n_b
                               void* d_workspace, void* stream)
 {
     (void)d_workspace;
-    if (!p || !d_spectrum || n_batch < 1) return FDAS_E_INVALID;
+    if (!p || !d_spectrum || n_batch < 1 || n_batch > 65535) return FDAS_E_INVALID;      // batch = gridDim.z
     if (!d_plane && !d_cands) return FDAS_E_INVALID;
     if (d_cands && !d_counts) return FDAS_E_INVALID;
     if (misaligned(d_spectrum, 8) || misaligned(d_plane, 16) || misaligned(d_cands, 4) || misaligned(d_counts, 4))
@@ -172,6 +179,7 @@ extern "C" int fdas_harmsum(fdas_plan* p, const float* d_plane, int32_t max_harm
 {
     if (!p || !d_plane || !h_thresholds || !d_cands || !d_count) return FDAS_E_INVALID;
     if (!valid_max_harm(max_harm) || p->interbin) return FDAS_E_INVALID;
+    if (!p->built) return FDAS_E_STATE;
     if (misaligned(d_plane, 4) || misaligned(d_cands, 4) || misaligned(d_count, 4)) return FDAS_E_INVALID;
     return fdas_launch_harmsum(p, d_plane, max_harm, h_thresholds, d_cands, d_count, capacity, (cudaStream_t)stream);
 }

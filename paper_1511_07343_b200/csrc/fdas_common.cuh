@@ -11,6 +11,8 @@ struct fdas_plan {
     double  z_max, dz;
     int32_t max_batch, quad_points;
     int32_t built;
+    // tuning keys (FDAS_OPT_TUNE_*; 0 = default), read by the launchers
+    int32_t tune_scalar, tune_t_chunks, tune_hs_sectors, tune_hs_rows, tune_hs_variant;
     // big FFT split of the packed half-length transform: M = n_samples/2 = R1*R2
     int32_t M, R1, R2, C1, C2, n_part;
     size_t  ws_inter_bytes, ws_part_bytes, workspace_bytes;
@@ -78,13 +80,28 @@ __device__ __forceinline__ float2 twiddle(int num, int den, float sign)
 }
 
 // Append one candidate; the slot counter receives the true count (include/fdas.h).
-__device__ __forceinline__ void push_cand(fdas_cand* list, uint32_t* count, uint32_t cap,
-                                          int col, int zi, int nharm, float power)
+__device__ __forceinline__ void store_cand(fdas_cand* list, uint32_t slot, uint32_t cap, int col, int zi, int nharm, float power)
 {
-    uint32_t slot = atomicAdd(count, 1u);
     if (slot < cap) {
         fdas_cand c;
         c.col = col; c.zi = (int16_t)zi; c.nharm = (int16_t)nharm; c.power = power;
         list[slot] = c;
     }
+}
+
+// Warp-ballot compaction: called by ALL 32 lanes of a converged warp, each with its own
+// predicate.  One ballot, ONE atomicAdd per warp (by the first lane that has a hit) for the warp's whole group
+// of records, the base handed round with a shuffle, lane-rank offsets inside the group.  The counter still
+// receives the true number found; records beyond `cap` are dropped.
+__device__ __forceinline__ void push_cand_warp(fdas_cand* list, uint32_t* count, uint32_t cap, bool hit,
+                                               int col, int zi, int nharm, float power)
+{
+    const unsigned m = __ballot_sync(0xffffffffu, hit);
+    if (m == 0) return;                                                  // warp-uniform
+    const unsigned lane = (threadIdx.x + threadIdx.y * blockDim.x) & 31u;
+    const int leader = __ffs((int)m) - 1;
+    uint32_t base = 0;
+    if ((int)lane == leader) base = atomicAdd(count, (uint32_t)__popc(m));
+    base = __shfl_sync(0xffffffffu, base, leader);
+    if (hit) store_cand(list, base + (uint32_t)__popc(m & ((1u << lane) - 1u)), cap, col, zi, nharm, power);
 }

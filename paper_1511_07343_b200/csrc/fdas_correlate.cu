@@ -5,9 +5,8 @@
 #include "fdas_common.cuh"
 #include "fdas_smemfft.cuh"
 #include "fdas_regfft.cuh"
-#include <stdlib.h>
 
-// v0 (generic L, natural-order smem Stockham): one CTA per (segment, batch entry).
+// Generic segment length (L != 2048; natural-order smem Stockham): one CTA per (segment, batch entry).
 // smem: X[L] | A[L] | B[L].
 __global__ void __launch_bounds__(256)
 k_correlate_smem(const float2* __restrict__ spec, const float2* __restrict__ W, float* __restrict__ plane,
@@ -37,49 +36,107 @@ k_correlate_smem(const float2* __restrict__ spec, const float2* __restrict__ W, 
         for (int i = threadIdx.x; i < L; i += blockDim.x) A[i] = cmul(X[i], Wt[i]);
         float2* y = smem_fft(A, B, L, 1, L, +1.0f);
         const int zi = t / nset, s = t - zi * nset;
-        for (int o = threadIdx.x; o < nvalid; o += blockDim.x) {
-            float2 v = y[o];
+        for (int o0 = 0; o0 < nvalid; o0 += blockDim.x) {                 // every warp stays converged (ballot below)
+            const int o = o0 + threadIdx.x;
+            const bool in = o < nvalid;
+            float2 v = in ? y[o] : make_float2(0.f, 0.f);
             float pw = fmaf(v.x, v.x, v.y * v.y);
             int col = (c0 + o) * nset + s;
-            if (plane) plane[((size_t)bt * n_z + zi) * n_cols + col] = pw;
-            if (cands && pw > thr) push_cand(cands + (size_t)bt * cap, counts + bt, cap, col, zi, 1, pw);
+            if (plane && in) plane[((size_t)bt * n_z + zi) * n_cols + col] = pw;
+            if (cands) push_cand_warp(cands + (size_t)bt * cap, counts + bt, cap, in && pw > thr, col, zi, 1, pw);
         }
     }
 }
 
 
 // ---------------------------------------------------------------------------------------------
-// v1, L = 2048: register-resident 16 x 16 x 8 FFTs, 128 threads (4 warps) per CTA, 16 points per
+// L = 2048: register-resident 16 x 16 x 8 FFTs, 128 threads (4 warps) per CTA, 16 points per
 // thread.  Index split (inverse, DIT):  k = 128 k1 + 8 k2 + k3,  t = t1 + 16 t2 + 256 t3:
 //   pass 1  thread (k2,k3): Y[k1] = X[k1] W[k1], 16-point DFT over k1 -> t1          (no twiddles)
-//   ex1     [k3][t1][k2] (pitch 17), intra-warp (a warp owns two k3 values)
+//   ex1     [k3][t1][k2], intra-warp (a warp owns two k3 values)
 //   pass 2  thread (t1,k3): twiddle exp(2 pi i k2 t1/256), 16-point DFT over k2 -> t2
 //   ex2     [k3][t2][t1], block barrier
-//   pass 3  thread p = t1 + 16 t2 (two per thread): twiddle exp(2 pi i k3 p/2048), 8-point DFT
+//   pass 3  two adjacent outputs p per thread: twiddle exp(2 pi i k3 p/2048), 8-point DFT
 //           over k3 -> t3;  |.|^2;  coalesced store of t = p + 256 t3 < step.
 // The forward transform of the window runs the same passes in reverse (once per segment) and
 // leaves X[128 k1 + 8 k2 + k3] in the registers pass 1 needs; the template spectra are stored
 // in that same register layout (Wr), so nothing is reordered in the template loop.
 // The segment spectrum X stays in registers across all templates ("data reuse").
-constexpr int V1_THREADS = 128;
-constexpr int V1_PITCH3 = 272;                 // float2 per k3 region: 16 rows of pitch 17
-constexpr int V1_BUF = 8 * V1_PITCH3;          // one exchange buffer (2176 float2)
+constexpr int SEG_THREADS = 128;
 
-__device__ __noinline__ void push_cand_slow(fdas_cand* list, uint32_t* count, uint32_t cap,
-                                            int col, int zi, float power)
+// out of line: the fused-threshold append is rare (called by all 32 lanes of a warp, see push_cand_warp)
+__device__ __noinline__ void push_cand_seg(fdas_cand* list, uint32_t* count, uint32_t cap, bool hit,
+                                           int col, int zi, float power)
 {
-    push_cand(list, count, cap, col, zi, 1, power);
+    push_cand_warp(list, count, cap, hit, col, zi, 1, power);
 }
 
-template <bool HAS_PLANE, bool HAS_CANDS, int NSET>
-__global__ void __launch_bounds__(V1_THREADS, 3)
+// Instruction economy of the template loop (cuobjdump: see DESIGN.md section 6.1):
+//   * the template multiply is folded into the first butterfly stage (mul_first_stage16);
+//   * exchange 1 rows have pitch 18 float2 (16-byte aligned), so pass 2 reads its 16 inputs with
+//     8 LDS.128 (quarter-warp bank pattern 4 lo + 4 j: conflict-free);
+//   * pass 3 owns the ADJACENT outputs p = 2 tid, 2 tid + 1: 8 LDS.128 from exchange 2, and for
+//     integer-bin planes 8-byte stores of two neighbouring columns;
+//   * PK: the butterflies use the packed f32x2 instructions of sm_100 (FFMA2/FADD2/FMUL2, fdas_regfft.cuh): the
+//     same operations per component in the same order (bit-identical planes), ~15 % fewer issue slots;
+//   * FAST (launched when step is a multiple of 256): a full segment keeps exactly t3 < step/256
+//     for every thread, so its stores are unpredicated and the butterflies feeding the discarded
+//     t3 = 7 outputs are dead code; the ragged last segment takes the predicated path.
+constexpr int SEG_PITCH3 = 288;                 // float2 per k3 region: 16 rows of pitch 18
+constexpr int SEG_BUF = 8 * SEG_PITCH3;
+
+// Pass 3 of one template for this thread's outputs p = 2 tid (u0) and 2 tid + 1 (u1), t = p + 256 t3:
+// 8 LDS.128 from exchange 2, two 8-point DITs over k3, |.|^2, store / threshold.
+// FULL (CTA-uniform): every thread keeps exactly t3 < NKEEP, so nothing is predicated and the work
+// feeding t3 >= NKEEP is dead code; otherwise t3 < nv (ragged last segment, or step not a multiple of 256).
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool FULL, bool PK>
+__device__ __forceinline__ void seg_pass3(const float2* buf, const float2* tw_a, const float2* tw_b, int tid,
+                                         float* prow, int nv, fdas_cand* cands, uint32_t* counts, uint32_t cap,
+                                         float thr, int col0, int zi)
+{
+    float2 u0[8], u1[8];
+#pragma unroll
+    for (int k3 = 0; k3 < 8; k3++) {
+        const float4 q = *reinterpret_cast<const float4*>(buf + 2 * tid + SEG_PITCH3 * k3);
+        u0[bitrev(k3, 3)] = make_float2(q.x, q.y);
+        u1[bitrev(k3, 3)] = make_float2(q.z, q.w);
+    }
+    dit_tw<8, PK>(u0, tw_a);
+    dit_tw<8, PK>(u1, tw_b);
+    float pa[8], pb[8];
+    float mx = 0.0f;                                   // largest kept power of this thread (fused threshold: one test)
+#pragma unroll
+    for (int t3 = 0; t3 < 8; t3++) {
+        if (FULL && t3 >= NKEEP) continue;             // compile time: the butterflies feeding these outputs are dead code
+        const bool kept = FULL || t3 < nv;
+        pa[t3] = fmaf(u0[t3].x, u0[t3].x, u0[t3].y * u0[t3].y);
+        pb[t3] = fmaf(u1[t3].x, u1[t3].x, u1[t3].y * u1[t3].y);
+        if (HAS_PLANE && kept) {
+            if (NSET == 1) *reinterpret_cast<float2*>(prow + 256 * t3) = make_float2(pa[t3], pb[t3]);
+            else { prow[(256 * t3) * NSET] = pa[t3]; prow[(256 * t3 + 1) * NSET] = pb[t3]; }
+        }
+        if (HAS_CANDS && kept) mx = fmaxf(mx, fmaxf(pa[t3], pb[t3]));
+    }
+    if (HAS_CANDS && __any_sync(0xffffffffu, mx > thr)) {      // rare; warp-uniform, so the ballots below see all 32 lanes
+#pragma unroll
+        for (int t3 = 0; t3 < 8; t3++) {
+            if (FULL && t3 >= NKEEP) continue;
+            const bool kept = FULL || t3 < nv;
+            push_cand_seg(cands, counts, cap, kept && pa[t3] > thr, col0 + 256 * t3 * NSET, zi, pa[t3]);
+            push_cand_seg(cands, counts, cap, kept && pb[t3] > thr, col0 + (256 * t3 + 1) * NSET, zi, pb[t3]);
+        }
+    }
+}
+
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK>
+__global__ void __launch_bounds__(SEG_THREADS, 3)
 k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
-                 fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
-                 int n_bins, int n_z, int m, int step, int t_chunk)
+                    fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
+                    int n_bins, int n_z, int m, int step, int t_chunk)
 {
     constexpr int L = 2048;
     constexpr int nset = NSET;
-    __shared__ float2 sm[2 * V1_BUF];
+    __shared__ __align__(16) float2 sm[2 * SEG_BUF];
     const int tid = threadIdx.x;
     const int lo = tid & 15, k3A = tid >> 4;
     const int seg = blockIdx.x, bt = blockIdx.z;
@@ -100,207 +157,26 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
                 long long c = (long long)c0 - m / 2 + p + 256 * n3;
                 u[bitrev(n3, 3)] = (c >= 0 && c < n_bins) ? S[c] : make_float2(0.f, 0.f);
             }
-            dit_const<8, -1>(u);
-#pragma unroll
-            for (int k3 = 0; k3 < 8; k3++) {
-                float2 val = k3 ? cmul(u[k3], twiddle(k3 * p, L, -1.0f)) : u[0];
-                buf[p + V1_PITCH3 * k3] = val;
-            }
-        }
-        __syncthreads();
-        float2 v[16];
-#pragma unroll
-        for (int n2 = 0; n2 < 16; n2++) v[bitrev(n2, 4)] = buf[lo + 16 * n2 + V1_PITCH3 * k3A];
-        dit_const<16, -1>(v);
-#pragma unroll
-        for (int k2 = 1; k2 < 16; k2++) v[k2] = cmul(v[k2], twiddle(k2 * lo, 256, -1.0f));
-        __syncwarp();
-#pragma unroll
-        for (int k2 = 0; k2 < 16; k2++) buf[k2 + 17 * lo + V1_PITCH3 * k3A] = v[k2];
-        __syncwarp();
-#pragma unroll
-        for (int n1 = 0; n1 < 16; n1++) v[bitrev(n1, 4)] = buf[lo + 17 * n1 + V1_PITCH3 * k3A];
-        dit_const<16, -1>(v);
-#pragma unroll
-        for (int k1 = 0; k1 < 16; k1++) X[k1] = v[k1];
-        __syncthreads();
-    }
-
-    // per-thread twiddles of the inverse passes (loop invariant)
-    float2 tw2[8], tw3[2][4];
-    make_tw<16>(tw2, lo, 256);
-    make_tw<8>(tw3[0], tid, L);
-    make_tw<8>(tw3[1], tid + 128, L);
-
-    const size_t n_cols = (size_t)n_bins * nset;
-    // number of kept outputs t = p + 256 t3 < min(step, n_bins - c0) for this thread's two p values
-    const int omax = min(step, n_bins - c0);
-    int nv[2];
-#pragma unroll
-    for (int g = 0; g < 2; g++) nv[g] = max(0, min(8, (omax - (tid + 128 * g) + 255) >> 8));
-    float* pbase = HAS_PLANE ? plane + (size_t)bt * n_z * n_cols + (size_t)(c0 + tid) * nset : nullptr;
-
-    // template spectra are software-pipelined: W(t+1) is fetched while pass 3 of template t runs
-    float4 w4[8];
-    if (t_begin < t_end) {
-        const float4* Wt = Wr + (size_t)t_begin * (8 * V1_THREADS) + tid;
-#pragma unroll
-        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wt + j * V1_THREADS);
-    }
-    for (int t = t_begin; t < t_end; t++) {
-        float2* buf = sm + ((t - t_begin) & 1) * V1_BUF;
-        float2 v[16];
-#pragma unroll
-        for (int j = 0; j < 8; j++) {
-            v[bitrev(2 * j, 4)] = cmul(X[2 * j], make_float2(w4[j].x, w4[j].y));
-            v[bitrev(2 * j + 1, 4)] = cmul(X[2 * j + 1], make_float2(w4[j].z, w4[j].w));
-        }
-        dit_const<16, +1>(v);                                                    // pass 1: k1 -> t1
-#pragma unroll
-        for (int t1 = 0; t1 < 16; t1++) buf[lo + 17 * t1 + V1_PITCH3 * k3A] = v[t1];
-        __syncwarp();
-#pragma unroll
-        for (int k2 = 0; k2 < 16; k2++) v[bitrev(k2, 4)] = buf[k2 + 17 * lo + V1_PITCH3 * k3A];
-        dit_tw<16>(v, tw2);                                                      // pass 2: k2 -> t2
-        __syncwarp();
-#pragma unroll
-        for (int t2 = 0; t2 < 16; t2++) buf[lo + 16 * t2 + V1_PITCH3 * k3A] = v[t2];
-        {
-            const float4* Wn = Wr + (size_t)min(t + 1, t_end - 1) * (8 * V1_THREADS) + tid;
-#pragma unroll
-            for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * V1_THREADS);
-        }
-        __syncthreads();
-        const int zi = NSET == 1 ? t : (t >> 1), s = NSET == 1 ? 0 : (t & 1);
-        float* prow = HAS_PLANE ? pbase + (size_t)zi * n_cols + s : nullptr;
-#pragma unroll
-        for (int g = 0; g < 2; g++) {
-            const int p = tid + 128 * g;
-            float2 u[8];
-#pragma unroll
-            for (int k3 = 0; k3 < 8; k3++) u[bitrev(k3, 3)] = buf[p + V1_PITCH3 * k3];
-            dit_tw<8>(u, tw3[g]);                                                // pass 3: k3 -> t3
-#pragma unroll
-            for (int t3 = 0; t3 < 8; t3++) {
-                float pw = fmaf(u[t3].x, u[t3].x, u[t3].y * u[t3].y);
-                if (t3 < nv[g]) {
-                    if (HAS_PLANE) prow[(128 * g + 256 * t3) * NSET] = pw;
-                    if (HAS_CANDS) {
-                        if (pw > thr)
-                            push_cand_slow(cands + (size_t)bt * cap, counts + bt, cap, (c0 + p + 256 * t3) * nset + s, zi, pw);
-                    }
-                }
-            }
-        }
-    }
-}
-
-// ---------------------------------------------------------------------------------------------
-// v2, L = 2048: same 16 x 16 x 8 register-resident scheme and index split as v1, with fewer
-// instructions per (segment, template) in the loop (cuobjdump: see DESIGN.md section 6.1):
-//   * the template multiply is folded into the first butterfly stage (mul_first_stage16);
-//   * exchange 1 rows have pitch 18 float2 (16-byte aligned), so pass 2 reads its 16 inputs with
-//     8 LDS.128 (quarter-warp bank pattern 4 lo + 4 j: conflict-free);
-//   * pass 3 owns the ADJACENT outputs p = 2 tid, 2 tid + 1: 8 LDS.128 from exchange 2, and for
-//     integer-bin planes 8-byte stores of two neighbouring columns;
-//   * PK: the butterflies use the packed f32x2 instructions of sm_100 (FFMA2/FADD2/FMUL2, fdas_regfft.cuh): the
-//     same operations per component in the same order (bit-identical planes), ~15 % fewer issue slots;
-//   * FAST (launched when step is a multiple of 256): a full segment keeps exactly t3 < step/256
-//     for every thread, so its stores are unpredicated and the butterflies feeding the discarded
-//     t3 = 7 outputs are dead code; the ragged last segment takes the predicated path.
-constexpr int V2_PITCH3 = 288;                 // float2 per k3 region: 16 rows of pitch 18
-constexpr int V2_BUF = 8 * V2_PITCH3;
-
-// Pass 3 of one template for this thread's outputs p = 2 tid (u0) and 2 tid + 1 (u1), t = p + 256 t3:
-// 8 LDS.128 from exchange 2, two 8-point DITs over k3, |.|^2, store / threshold.
-// FULL (CTA-uniform): every thread keeps exactly t3 < NKEEP, so nothing is predicated and the work
-// feeding t3 >= NKEEP is dead code; otherwise t3 < nv (ragged last segment, or step not a multiple of 256).
-template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool FULL, bool PK>
-__device__ __forceinline__ void v2_pass3(const float2* buf, const float2* tw_a, const float2* tw_b, int tid,
-                                         float* prow, int nv, fdas_cand* cands, uint32_t* counts, uint32_t cap,
-                                         float thr, int col0, int zi)
-{
-    float2 u0[8], u1[8];
-#pragma unroll
-    for (int k3 = 0; k3 < 8; k3++) {
-        const float4 q = *reinterpret_cast<const float4*>(buf + 2 * tid + V2_PITCH3 * k3);
-        u0[bitrev(k3, 3)] = make_float2(q.x, q.y);
-        u1[bitrev(k3, 3)] = make_float2(q.z, q.w);
-    }
-    dit_tw<8, PK>(u0, tw_a);
-    dit_tw<8, PK>(u1, tw_b);
-    float pa[8], pb[8];
-    float mx = 0.0f;                                   // largest kept power of this thread (fused threshold: one test)
-#pragma unroll
-    for (int t3 = 0; t3 < 8; t3++) {
-        if (FULL ? (t3 >= NKEEP) : (t3 >= nv)) continue;
-        pa[t3] = fmaf(u0[t3].x, u0[t3].x, u0[t3].y * u0[t3].y);
-        pb[t3] = fmaf(u1[t3].x, u1[t3].x, u1[t3].y * u1[t3].y);
-        if (HAS_PLANE) {
-            if (NSET == 1) *reinterpret_cast<float2*>(prow + 256 * t3) = make_float2(pa[t3], pb[t3]);
-            else { prow[(256 * t3) * NSET] = pa[t3]; prow[(256 * t3 + 1) * NSET] = pb[t3]; }
-        }
-        if (HAS_CANDS) mx = fmaxf(mx, fmaxf(pa[t3], pb[t3]));
-    }
-    if (HAS_CANDS && mx > thr) {                       // rare
-#pragma unroll
-        for (int t3 = 0; t3 < 8; t3++) {
-            if (FULL ? (t3 >= NKEEP) : (t3 >= nv)) continue;
-            if (pa[t3] > thr) push_cand_slow(cands, counts, cap, col0 + 256 * t3 * NSET, zi, pa[t3]);
-            if (pb[t3] > thr) push_cand_slow(cands, counts, cap, col0 + (256 * t3 + 1) * NSET, zi, pb[t3]);
-        }
-    }
-}
-
-template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK>
-__global__ void __launch_bounds__(V1_THREADS, 3)
-k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
-                    fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
-                    int n_bins, int n_z, int m, int step, int t_chunk)
-{
-    constexpr int L = 2048;
-    constexpr int nset = NSET;
-    __shared__ __align__(16) float2 sm[2 * V2_BUF];
-    const int tid = threadIdx.x;
-    const int lo = tid & 15, k3A = tid >> 4;
-    const int seg = blockIdx.x, bt = blockIdx.z;
-    const int n_t = n_z * nset;
-    const int t_begin = blockIdx.y * t_chunk, t_end = min(n_t, t_begin + t_chunk);
-    const int c0 = seg * step;
-    const float2* S = spec + (size_t)bt * n_bins;
-
-    float2 X[16];
-    {   // ---- forward FFT of the window (sign -), reverse pass order (as v1)
-        float2* buf = sm;
-#pragma unroll
-        for (int g = 0; g < 2; g++) {
-            const int p = tid + 128 * g;
-            float2 u[8];
-#pragma unroll
-            for (int n3 = 0; n3 < 8; n3++) {
-                long long c = (long long)c0 - m / 2 + p + 256 * n3;
-                u[bitrev(n3, 3)] = (c >= 0 && c < n_bins) ? S[c] : make_float2(0.f, 0.f);
-            }
             dit_const<8, -1, PK>(u);
 #pragma unroll
             for (int k3 = 0; k3 < 8; k3++) {
                 float2 val = k3 ? cmul(u[k3], twiddle(k3 * p, L, -1.0f)) : u[0];
-                buf[p + V2_PITCH3 * k3] = val;
+                buf[p + SEG_PITCH3 * k3] = val;
             }
         }
         __syncthreads();
         float2 v[16];
 #pragma unroll
-        for (int n2 = 0; n2 < 16; n2++) v[bitrev(n2, 4)] = buf[lo + 16 * n2 + V2_PITCH3 * k3A];
+        for (int n2 = 0; n2 < 16; n2++) v[bitrev(n2, 4)] = buf[lo + 16 * n2 + SEG_PITCH3 * k3A];
         dit_const<16, -1, PK>(v);
 #pragma unroll
         for (int k2 = 1; k2 < 16; k2++) v[k2] = cmul(v[k2], twiddle(k2 * lo, 256, -1.0f));
         __syncwarp();
 #pragma unroll
-        for (int k2 = 0; k2 < 16; k2++) buf[k2 + 18 * lo + V2_PITCH3 * k3A] = v[k2];
+        for (int k2 = 0; k2 < 16; k2++) buf[k2 + 18 * lo + SEG_PITCH3 * k3A] = v[k2];
         __syncwarp();
 #pragma unroll
-        for (int n1 = 0; n1 < 16; n1++) v[bitrev(n1, 4)] = buf[lo + 18 * n1 + V2_PITCH3 * k3A];
+        for (int n1 = 0; n1 < 16; n1++) v[bitrev(n1, 4)] = buf[lo + 18 * n1 + SEG_PITCH3 * k3A];
         dit_const<16, -1, PK>(v);
 #pragma unroll
         for (int k1 = 0; k1 < 16; k1++) X[k1] = v[k1];
@@ -321,14 +197,14 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
     uint32_t* ccount = HAS_CANDS ? counts + bt : nullptr;
 
     float4 w4[8];
-    const float4* Wn = Wr + (size_t)t_begin * (8 * V1_THREADS) + tid;      // template whose spectrum is fetched next
+    const float4* Wn = Wr + (size_t)t_begin * (8 * SEG_THREADS) + tid;      // template whose spectrum is fetched next
     if (t_begin < t_end) {
 #pragma unroll
-        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * V1_THREADS);
+        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * SEG_THREADS);
     }
     float* prow1 = HAS_PLANE ? pbase + (size_t)t_begin * n_cols : nullptr;  // NSET == 1: row of template t
     for (int t = t_begin; t < t_end; t++) {
-        float2* buf = sm + ((t - t_begin) & 1) * V2_BUF;
+        float2* buf = sm + ((t - t_begin) & 1) * SEG_BUF;
         float2 v[16];
         if (PK) mul_first_stage16_pk(v, X, w4);                                  // X W and stage 1
         else mul_first_stage16(v, X, w4);
@@ -336,10 +212,10 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
         dit_const_stage<16, +1, 3, PK>(v);
         dit_const_stage<16, +1, 4, PK>(v);
 #pragma unroll
-        for (int t1 = 0; t1 < 16; t1++) buf[lo + 18 * t1 + V2_PITCH3 * k3A] = v[t1];
+        for (int t1 = 0; t1 < 16; t1++) buf[lo + 18 * t1 + SEG_PITCH3 * k3A] = v[t1];
         __syncwarp();
         {
-            const float4* row = reinterpret_cast<const float4*>(buf + 18 * lo + V2_PITCH3 * k3A);
+            const float4* row = reinterpret_cast<const float4*>(buf + 18 * lo + SEG_PITCH3 * k3A);
 #pragma unroll
             for (int j = 0; j < 8; j++) {
                 const float4 q = row[j];
@@ -350,19 +226,19 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
         dit_tw<16, PK>(v, tw2);                                                  // pass 2: k2 -> t2
         __syncwarp();
 #pragma unroll
-        for (int t2 = 0; t2 < 16; t2++) buf[lo + 16 * t2 + V2_PITCH3 * k3A] = v[t2];
-        if (t + 1 < t_end) Wn += 8 * V1_THREADS;                                 // (the last iteration re-reads its own)
+        for (int t2 = 0; t2 < 16; t2++) buf[lo + 16 * t2 + SEG_PITCH3 * k3A] = v[t2];
+        if (t + 1 < t_end) Wn += 8 * SEG_THREADS;                                 // (the last iteration re-reads its own)
 #pragma unroll
-        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * V1_THREADS);
+        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * SEG_THREADS);
         __syncthreads();
         const int zi = NSET == 1 ? t : (t >> 1), s = NSET == 1 ? 0 : (t & 1);
         float* prow = !HAS_PLANE ? nullptr : NSET == 1 ? prow1 : pbase + (size_t)zi * n_cols + s;
         if (HAS_PLANE && NSET == 1) prow1 += n_cols;
         const int col0 = (c0 + 2 * tid) * nset + s;
         if (full)                                                                // pass 3: k3 -> t3
-            v2_pass3<HAS_PLANE, HAS_CANDS, NSET, NKEEP, true, PK>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
+            seg_pass3<HAS_PLANE, HAS_CANDS, NSET, NKEEP, true, PK>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
         else
-            v2_pass3<HAS_PLANE, HAS_CANDS, NSET, 8, false, PK>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
+            seg_pass3<HAS_PLANE, HAS_CANDS, NSET, 8, false, PK>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
     }
 }
 
@@ -370,8 +246,8 @@ k_correlate_2048_v2(const float2* __restrict__ spec, const float4* __restrict__ 
 __global__ void k_permute_templates_2048(const float2* __restrict__ W, float4* __restrict__ Wr, int n_t)
 {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= n_t * 8 * V1_THREADS) return;
-    int tid = i % V1_THREADS, j = (i / V1_THREADS) % 8, t = i / (8 * V1_THREADS);
+    if (i >= n_t * 8 * SEG_THREADS) return;
+    int tid = i % SEG_THREADS, j = (i / SEG_THREADS) % 8, t = i / (8 * SEG_THREADS);
     int k2 = tid & 15, k3 = tid >> 4;
     float2 a = W[(size_t)t * 2048 + 128 * (2 * j) + 8 * k2 + k3];
     float2 b = W[(size_t)t * 2048 + 128 * (2 * j + 1) + 8 * k2 + k3];
@@ -381,7 +257,7 @@ __global__ void k_permute_templates_2048(const float2* __restrict__ W, float4* _
 int fdas_permute_templates(fdas_plan* p, cudaStream_t st)
 {
     if (p->L != 2048) return FDAS_OK;
-    int n = p->n_t * 8 * V1_THREADS;
+    int n = p->n_t * 8 * SEG_THREADS;
     k_permute_templates_2048<<<(n + 255) / 256, 256, 0, st>>>(p->d_W, reinterpret_cast<float4*>(p->d_Wr), p->n_t);
     FDAS_LAUNCH_CHECK();
     return FDAS_OK;
@@ -391,38 +267,32 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
                           fdas_cand* d_cands, uint32_t* d_counts, uint32_t cap, cudaStream_t st)
 {
     if (d_cands) FDAS_CUDA(cudaMemsetAsync(d_counts, 0, sizeof(uint32_t) * n_batch, st));
-    const bool force_v0 = getenv("FDAS_CORRELATE_V0") != nullptr;
-    if (p->L == 2048 && !force_v0) {
-        const int env_chunks = getenv("FDAS_T_CHUNKS") ? atoi(getenv("FDAS_T_CHUNKS")) : 0;
-        int n_chunk = env_chunks > 0 ? env_chunks : (p->n_t + 28) / 29;      // ~29 templates per CTA: short tail
+    if (p->L == 2048) {
+        int n_chunk = p->tune_t_chunks > 0 ? p->tune_t_chunks : (p->n_t + 28) / 29;      // ~29 templates per CTA: short tail
         int t_chunk = (p->n_t + n_chunk - 1) / n_chunk;
         n_chunk = (p->n_t + t_chunk - 1) / t_chunk;
         dim3 grid(p->n_seg, n_chunk, n_batch);
-#define FDAS_V1_ARGS d_spec, reinterpret_cast<const float4*>(p->d_Wr), d_plane, d_cands, d_counts, cap, thr, \
-                     (int)p->n_bins, p->n_z, p->m, p->step, t_chunk
-#define FDAS_V1_LAUNCH(K, ...)                                                                      \
-        if (d_plane && d_cands) K<true, true, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS); \
-        else if (d_plane) K<true, false, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS);      \
-        else K<false, true, __VA_ARGS__><<<grid, V1_THREADS, 0, st>>>(FDAS_V1_ARGS)
-        // tuning switches, read at every call (a few hundred ns) so that one process can time the variants
-        const bool use_v1 = getenv("FDAS_CORRELATE_V1") != nullptr;
-        const bool scalar = getenv("FDAS_CORRELATE_SCALAR") != nullptr;     // v2 with scalar FFMA butterflies
+#define FDAS_SEG_ARGS d_spec, reinterpret_cast<const float4*>(p->d_Wr), d_plane, d_cands, d_counts, cap, thr, \
+                      (int)p->n_bins, p->n_z, p->m, p->step, t_chunk
+#define FDAS_SEG_LAUNCH(...)                                                                                        \
+        if (d_plane && d_cands) k_correlate_2048<true, true, __VA_ARGS__><<<grid, SEG_THREADS, 0, st>>>(FDAS_SEG_ARGS); \
+        else if (d_plane) k_correlate_2048<true, false, __VA_ARGS__><<<grid, SEG_THREADS, 0, st>>>(FDAS_SEG_ARGS);      \
+        else k_correlate_2048<false, true, __VA_ARGS__><<<grid, SEG_THREADS, 0, st>>>(FDAS_SEG_ARGS)
+        const bool scalar = p->tune_scalar != 0;                  // scalar FFMA butterflies (tuning key; bit-identical planes)
         const bool keep7 = p->step == 7 * 256;                    // m = 256: full segments keep t3 < 7 exactly
-#define FDAS_V2_LAUNCH(NS)                                                                                        \
-        if (keep7 && !scalar) { FDAS_V1_LAUNCH(k_correlate_2048_v2, NS, 7, true); }                               \
-        else if (keep7) { FDAS_V1_LAUNCH(k_correlate_2048_v2, NS, 7, false); }                                    \
-        else if (!scalar) { FDAS_V1_LAUNCH(k_correlate_2048_v2, NS, 8, true); }                                   \
-        else { FDAS_V1_LAUNCH(k_correlate_2048_v2, NS, 8, false); }
-        if (use_v1) {
-            if (p->nset == 1) { FDAS_V1_LAUNCH(k_correlate_2048, 1); } else { FDAS_V1_LAUNCH(k_correlate_2048, 2); }
-        } else if (p->nset == 1) {
-            FDAS_V2_LAUNCH(1)
+#define FDAS_SEG_LAUNCH_NS(NS)                                                                   \
+        if (keep7 && !scalar) { FDAS_SEG_LAUNCH(NS, 7, true); }                                  \
+        else if (keep7) { FDAS_SEG_LAUNCH(NS, 7, false); }                                       \
+        else if (!scalar) { FDAS_SEG_LAUNCH(NS, 8, true); }                                      \
+        else { FDAS_SEG_LAUNCH(NS, 8, false); }
+        if (p->nset == 1) {
+            FDAS_SEG_LAUNCH_NS(1)
         } else {
-            FDAS_V2_LAUNCH(2)
+            FDAS_SEG_LAUNCH_NS(2)
         }
-#undef FDAS_V2_LAUNCH
-#undef FDAS_V1_LAUNCH
-#undef FDAS_V1_ARGS
+#undef FDAS_SEG_LAUNCH_NS
+#undef FDAS_SEG_LAUNCH
+#undef FDAS_SEG_ARGS
         FDAS_LAUNCH_CHECK();
         return FDAS_OK;
     }

@@ -1,7 +1,7 @@
 // fdas_harmsum.cu -- incoherent harmonic summing and candidate compaction
 // (BASELINE.json configs[4]; "pulse harmonics").
 #include "fdas_common.cuh"
-#include <stdlib.h>
+#include <math.h>
 
 struct HarmThr { float t[5]; };
 
@@ -17,10 +17,11 @@ struct HarmThr { float t[5]; };
 // grid = ceil(n_cols/(32 HS_CPT)), block = (32, 8).
 constexpr int HS_ROWS_PER_PASS = 8;
 
-__device__ __noinline__ void push_cand_hs(fdas_cand* list, uint32_t* count, uint32_t cap,
+// out of line: rare (called by all 32 lanes of a warp, see push_cand_warp)
+__device__ __noinline__ void push_cand_hs(fdas_cand* list, uint32_t* count, uint32_t cap, bool hit,
                                           int col, int zi, int nharm, float power)
 {
-    push_cand(list, count, cap, col, zi, nharm, power);
+    push_cand_warp(list, count, cap, hit, col, zi, nharm, power);
 }
 
 // CHECK = true: edge tiles (first tile: k_h may fall below bin0; last tile: columns beyond n_cols).
@@ -135,13 +136,13 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
                 sum[st] = acc;
                 any = any || acc.x > thr.t[st] || acc.y > thr.t[st];
             }
-            if (any) {
+            if (__any_sync(0xffffffffu, any)) {                         // warp-uniform: the ballots below see all 32 lanes
 #pragma unroll
                 for (int st = 0; st < NST; st++) {
-                    if (sum[st].x > thr.t[st] && (!CHECK || (okmask >> (2 * jj) & 1)))
-                        push_cand_hs(cands, count, cap, col0 + 32 * (2 * jj), zi, 1 << st, sum[st].x);
-                    if (sum[st].y > thr.t[st] && (!CHECK || (okmask >> (2 * jj + 1) & 1)))
-                        push_cand_hs(cands, count, cap, col0 + 32 * (2 * jj + 1), zi, 1 << st, sum[st].y);
+                    push_cand_hs(cands, count, cap, sum[st].x > thr.t[st] && (!CHECK || (okmask >> (2 * jj) & 1)),
+                                 col0 + 32 * (2 * jj), zi, 1 << st, sum[st].x);
+                    push_cand_hs(cands, count, cap, sum[st].y > thr.t[st] && (!CHECK || (okmask >> (2 * jj + 1) & 1)),
+                                 col0 + 32 * (2 * jj + 1), zi, 1 << st, sum[st].y);
                 }
             }
         }
@@ -253,8 +254,10 @@ static int resident_ctas(K k, int threads)
     return sms * per_sm;
 }
 
-// Threshold + compaction over one plane (row a8). grid-stride over float4 groups of a row.
-// grid = (ceil(n_cols/1024), n_z), block 256.
+// Threshold + warp-ballot compaction over one plane (row a8): a thread tests 4 adjacent columns of a row (one
+// 16-byte load where the address allows it -- the plane pointer itself need only be 4-byte aligned,
+// include/fdas.h -- else scalar loads); each of the 4 is appended with one ballot and one atomic per warp.
+// No thread leaves early: the ballots need the whole warp.   grid = (ceil(n_cols/1024), n_z), block 256.
 __global__ void __launch_bounds__(256)
 k_candidates(const float* __restrict__ plane, fdas_cand* __restrict__ cands, uint32_t* __restrict__ count,
              uint32_t cap, float thr, int n_cols)
@@ -262,19 +265,18 @@ k_candidates(const float* __restrict__ plane, fdas_cand* __restrict__ cands, uin
     const int zi = blockIdx.y;
     const float* row = plane + (size_t)zi * n_cols;
     const int c4 = (blockIdx.x * blockDim.x + threadIdx.x) * 4;
-    if (c4 >= n_cols) return;
-    if (c4 + 3 < n_cols && ((((size_t)zi * n_cols) & 3) == 0)) {
-        float4 v = __ldg(reinterpret_cast<const float4*>(row + c4));
-        if (v.x > thr) push_cand(cands, count, cap, c4, zi, 1, v.x);
-        if (v.y > thr) push_cand(cands, count, cap, c4 + 1, zi, 1, v.y);
-        if (v.z > thr) push_cand(cands, count, cap, c4 + 2, zi, 1, v.z);
-        if (v.w > thr) push_cand(cands, count, cap, c4 + 3, zi, 1, v.w);
+    float v[4] = {0.0f, 0.0f, 0.0f, 0.0f};
+    if (c4 + 3 < n_cols && (reinterpret_cast<uintptr_t>(row + c4) & 15) == 0) {
+        const float4 q = __ldg(reinterpret_cast<const float4*>(row + c4));
+        v[0] = q.x; v[1] = q.y; v[2] = q.z; v[3] = q.w;
     } else {
-        for (int c = c4; c < min(c4 + 4, n_cols); c++) {
-            float v = __ldg(row + c);
-            if (v > thr) push_cand(cands, count, cap, c, zi, 1, v);
-        }
+#pragma unroll
+        for (int i = 0; i < 4; i++)
+            if (c4 + i < n_cols) v[i] = __ldg(row + c4 + i);
     }
+#pragma unroll
+    for (int i = 0; i < 4; i++)
+        push_cand_warp(cands, count, cap, c4 + i < n_cols && v[i] > thr, c4 + i, zi, 1, v[i]);
 }
 
 int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const float* h_thr,
@@ -287,11 +289,11 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     for (int i = 0; i < 5; i++) thr.t[i] = i < n_stage ? h_thr[i] : 3.0e38f;
     FDAS_CUDA(cudaMemsetAsync(d_count, 0, sizeof(uint32_t), st));
     int n_cols = (int)p->n_cols;
-    const int variant = getenv("FDAS_HS_VARIANT") ? atoi(getenv("FDAS_HS_VARIANT")) : 0;
+    const int variant = p->tune_hs_variant;
     // sectors of the tile order (see k_harmsum): 16 by default, thin enough for the reuse distance to fit in
     // L2, thick enough (~10 rows at the far end) for L1 to keep serving the row-direction reuse inside a stream
-    const int env_sectors = getenv("FDAS_HS_SECTORS") ? atoi(getenv("FDAS_HS_SECTORS")) : 16;
-    const int env_rows = getenv("FDAS_HS_ROWS") ? atoi(getenv("FDAS_HS_ROWS")) : 0;
+    const int env_sectors = p->tune_hs_sectors > 0 ? p->tune_hs_sectors : 16;
+    const int env_rows = p->tune_hs_rows;
     int n_sec = env_sectors < 1 ? 1 : env_sectors;
     if (n_sec > HS_MAX_SECTORS) n_sec = HS_MAX_SECTORS;
     int rows = env_rows > 0 ? env_rows : (n_sec == 1 ? HS_ROWS_PER_PASS : 4);      // warps per CTA: with sectors, 4 adjacent column tiles (all rows of the

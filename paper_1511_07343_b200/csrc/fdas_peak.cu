@@ -50,36 +50,36 @@ k_ffma2_peak(float* __restrict__ sink, float x, float y, int iters)
     if (s == 123.456f) sink[0] = s;
 }
 
-extern "C" int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, void* stream)
+extern "C" int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, int32_t packed, void* stream)
 {
     if (!out_tflops) return FDAS_E_INVALID;
-    // out_ms, when given, carries the mode in: *out_ms < 0 on entry selects the packed FFMA2 chains
-    const bool packed = out_ms && *out_ms < 0.0;
     cudaStream_t st = (cudaStream_t)stream;
     int dev = 0, sms = 0;
     FDAS_CUDA(cudaGetDevice(&dev));
     FDAS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     float* sink = nullptr;
-    FDAS_CUDA(cudaMalloc(&sink, sizeof(float)));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
     const int iters = 4096, grid = sms * 8, block = 256;
-    cudaEvent_t e0, e1;
-    FDAS_CUDA(cudaEventCreate(&e0));
-    FDAS_CUDA(cudaEventCreate(&e1));
     double best_ms = 1.0e30;
-    for (int rep = 0; rep < 5; rep++) {                       // rep 0 warms up; best of the rest (burst figure)
-        FDAS_CUDA(cudaEventRecord(e0, st));
+    cudaError_t err = cudaMalloc(&sink, sizeof(float));
+    if (err == cudaSuccess) err = cudaEventCreate(&e0);
+    if (err == cudaSuccess) err = cudaEventCreate(&e1);
+    for (int rep = 0; rep < 5 && err == cudaSuccess; rep++) {   // rep 0 warms up; best of the rest (burst figure)
+        err = cudaEventRecord(e0, st);
+        if (err != cudaSuccess) break;
         if (packed) k_ffma2_peak<<<grid, block, 0, st>>>(sink, 0.999f, 1.0e-3f, iters);
         else k_ffma_peak<<<grid, block, 0, st>>>(sink, 0.999f, 1.0e-3f, iters);
-        FDAS_CUDA(cudaEventRecord(e1, st));
-        FDAS_CUDA(cudaEventSynchronize(e1));
-        FDAS_LAUNCH_CHECK();
+        err = cudaGetLastError();
+        if (err == cudaSuccess) err = cudaEventRecord(e1, st);
+        if (err == cudaSuccess) err = cudaEventSynchronize(e1);
         float ms = 0.0f;
-        FDAS_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-        if (rep > 0 && ms < best_ms) best_ms = ms;
+        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+        if (err == cudaSuccess && rep > 0 && ms < best_ms) best_ms = ms;
     }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
-    cudaFree(sink);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (sink) cudaFree(sink);
+    if (err != cudaSuccess) { fdas_set_cuda_error(err, "fdas_measure_fp32_tflops"); return FDAS_E_CUDA; }
     const double flops = 2.0 * 4.0 * PEAK_ACC * (double)iters * (double)grid * (double)block;
     *out_tflops = flops / (best_ms * 1.0e-3) / 1.0e12;
     if (out_ms) *out_ms = best_ms;

@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libfdas.so")
 
 FDAS_OK, FDAS_E_INVALID, FDAS_E_STATE, FDAS_E_WORKSPACE, FDAS_E_CUDA, FDAS_E_NOMEM = 0, -1, -2, -3, -4, -5
 FDAS_OPT_INTERBIN, FDAS_OPT_MAX_BATCH, FDAS_OPT_QUAD_POINTS = 1, 2, 3
+FDAS_OPT_TUNE_SCALAR, FDAS_OPT_TUNE_T_CHUNKS, FDAS_OPT_TUNE_HS_SECTORS, FDAS_OPT_TUNE_HS_ROWS, FDAS_OPT_TUNE_HS_VARIANT = 101, 102, 103, 104, 105
 
 CAND_DTYPE = np.dtype([("col", "<i4"), ("zi", "<i2"), ("nharm", "<i2"), ("power", "<f4")])
 assert CAND_DTYPE.itemsize == 12
@@ -65,7 +66,7 @@ def lib():
         L.fdas_candidates.argtypes = [vp, vp, f32, vp, vp, u32, vp]
         L.fdas_resample.argtypes = [vp, vp, f64, vp, vp]
         L.fdas_search_host.argtypes = [vp, vp, i32, i32, vp, vp, vp, u32, vp]
-        L.fdas_measure_fp32_tflops.argtypes = [C.POINTER(f64), C.POINTER(f64), vp]
+        L.fdas_measure_fp32_tflops.argtypes = [C.POINTER(f64), C.POINTER(f64), i32, vp]
         L.fdas_threshold.argtypes = [i32, f64]
         L.fdas_threshold.restype = f64
         L.fdas_plan_destroy.argtypes = [vp]
@@ -181,8 +182,9 @@ def fdas_threshold(n_harm: int, pfa: float = 1e-6) -> float:
 
 def fdas_measure_fp32_tflops(stream=None, packed=False):
     """(TFLOP/s, ms) of the FFMA-chain microbenchmark on the current device (packed: FFMA2 chains)."""
-    tf, ms = C.c_double(), C.c_double(-1.0 if packed else 0.0)
-    _check(lib().fdas_measure_fp32_tflops(C.byref(tf), C.byref(ms), _stream(stream)), "fdas_measure_fp32_tflops")
+    tf, ms = C.c_double(), C.c_double()
+    _check(lib().fdas_measure_fp32_tflops(C.byref(tf), C.byref(ms), 1 if packed else 0, _stream(stream)),
+           "fdas_measure_fp32_tflops")
     return tf.value, ms.value
 
 

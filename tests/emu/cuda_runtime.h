@@ -1,4 +1,4 @@
-// Host emulation shim for CUDA device code (dev tool, _work only).
+// Host emulation shim for CUDA device code: committed TEST INFRASTRUCTURE (tests/emu/README.md), never on the product path.
 #pragma once
 #include <math.h>
 #include <stdint.h>
@@ -60,11 +60,13 @@ template <class T> static inline cudaError_t cudaMallocHost(T** p, size_t n) { *
 static inline cudaError_t cudaFreeHost(void* p) { free(p); return cudaSuccess; }
 static inline cudaError_t cudaGetLastError() { return cudaSuccess; }
 static inline cudaError_t cudaSetDevice(int) { return cudaSuccess; }
-// a small pretend device: 3 SMs, 2 resident CTAs each (persistent kernels then loop over several items per CTA)
+// the pretend device: EMU_SMS SMs (default 3) with EMU_CTAS_PER_SM resident CTAs each (default 2), so that persistent
+// kernels loop over several items per CTA; EMU_SMS=148 with the real occupancy exercises the B200 geometry
 enum cudaDeviceAttr { cudaDevAttrMultiProcessorCount = 16 };
+int emu_env_int(const char* name, int dflt);
 static inline cudaError_t cudaGetDevice(int* d) { *d = 0; return cudaSuccess; }
-static inline cudaError_t cudaDeviceGetAttribute(int* v, cudaDeviceAttr, int) { *v = 3; return cudaSuccess; }
-template <class F> static inline cudaError_t cudaOccupancyMaxActiveBlocksPerMultiprocessor(int* n, F, int, size_t) { *n = 2; return cudaSuccess; }
+static inline cudaError_t cudaDeviceGetAttribute(int* v, cudaDeviceAttr, int) { *v = emu_env_int("EMU_SMS", 3); return cudaSuccess; }
+template <class F> static inline cudaError_t cudaOccupancyMaxActiveBlocksPerMultiprocessor(int* n, F, int, size_t) { *n = emu_env_int("EMU_CTAS_PER_SM", 2); return cudaSuccess; }
 static inline const char* cudaGetErrorString(cudaError_t) { return "emu"; }
 template <class F> static inline cudaError_t cudaFuncSetAttribute(F, cudaFuncAttribute, int) { return cudaSuccess; }
 
@@ -80,6 +82,15 @@ static inline unsigned __ballot_sync(unsigned mask, int pred)
     if (mask != 0xffffffffu) { fprintf(stderr, "EMU: __ballot_sync with a partial mask is not modelled\n"); abort(); }
     return emu_ballot(pred);
 }
+unsigned emu_shfl(unsigned v, int src_lane);
+static inline unsigned __shfl_sync(unsigned mask, unsigned v, int src_lane)
+{
+    if (mask != 0xffffffffu) { fprintf(stderr, "EMU: __shfl_sync with a partial mask is not modelled\n"); abort(); }
+    return emu_shfl(v, src_lane);
+}
+static inline int __any_sync(unsigned mask, int pred) { return __ballot_sync(mask, pred) != 0; }
+static inline int __ffs(int x) { return __builtin_ffs(x); }
+static inline int __popc(unsigned x) { return __builtin_popcount(x); }
 static inline int __clz(int x) { return x ? __builtin_clz((unsigned)x) : 32; }
 #define __syncthreads() emu_syncthreads()
 #define __syncwarp() emu_syncwarp()

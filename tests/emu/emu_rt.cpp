@@ -1,4 +1,4 @@
-// Host emulation runtime: guard-paged "device" memory + coroutine CTA scheduler (dev tool).
+// Host emulation runtime: guard-paged "device" memory + coroutine CTA scheduler (test infrastructure, tests/emu/README.md).
 #include "cuda_runtime.h"
 #include <signal.h>
 #include <sys/mman.h>
@@ -127,6 +127,7 @@ struct Fiber { Ctx ctx; char* stack; int state; uint3 tid; unsigned n_ballot; };
 struct Worker {
     std::vector<Fiber> fibers;
     std::vector<unsigned> ballot;            // [warp][2]: alternating accumulators of __ballot_sync
+    std::vector<unsigned> shfl;              // [thread]: the value each lane offers to __shfl_sync
     Ctx sched;
     int cur;
     const std::function<void()>* body;
@@ -170,6 +171,27 @@ unsigned emu_ballot(int pred)
     return r;
 }
 
+// __shfl_sync over the full warp: every lane publishes its value, warp barrier, read the source lane's,
+// warp barrier (so that nobody overwrites a slot that is still being read).
+unsigned emu_shfl(unsigned v, int src_lane)
+{
+    Worker* w = t_w;
+    const int i = w->cur, warp = i / 32;
+    w->shfl[i] = v;
+    yield_with(ST_WARP_BAR);
+    w = t_w;
+    const unsigned r = w->shfl[32 * warp + (src_lane & 31)];
+    yield_with(ST_WARP_BAR);
+    return r;
+}
+
+int emu_env_int(const char* name, int dflt)
+{
+    const char* e = getenv(name);
+    const int v = e ? atoi(e) : dflt;
+    return v > 0 ? v : dflt;
+}
+
 static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward, 1 reversed, >= 2 pseudo-random (seed)
 {
     const bool rev = order == 1;
@@ -189,6 +211,7 @@ static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward
         f.tid = uint3{(unsigned)i % block.x, ((unsigned)i / block.x) % block.y, (unsigned)i / (block.x * block.y)};
     }
     w->ballot.assign(2 * ((nt + 31) / 32), 0u);
+    w->shfl.assign(32 * ((nt + 31) / 32), 0u);
     int done = 0;
     while (done < nt) {
         bool progress = false;

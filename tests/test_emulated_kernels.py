@@ -191,36 +191,93 @@ def test_time_domain_trial_end_to_end(emu):
 
 
 def test_correlate_variants_agree(emu):
-    """The kernel variants kept for tuning (FDAS_* switches, read at every call): the packed f32x2 butterflies
-    give the scalar ones' plane bit for bit; the previous kernel (v1) and the generic shared-memory kernel
-    (v0) agree to rounding; the harmonic sum does not depend on its sector count."""
+    """The tuning keys (FDAS_OPT_TUNE_*) change instruction selection and launch geometry only: the packed f32x2
+    butterflies give the scalar ones' plane bit for bit, the number of template chunks per segment does not
+    matter, and the harmonic sum does not depend on its sector count, warps per CTA or tile width."""
     cfg = synth.small_config(1 << 13, 12.0, 2.0, 256, 2048, n_sig=2, index=7, amp=0.2)
     plan = emu.Plan(cfg.n_samples, cfg.z_max, cfg.dz, cfg.width, cfg.seg_len, quad_points=2048)
     d_S, _ = plan.spectrum(cfg.series())
     planes = {}
-    for name, env in (("packed", {}), ("scalar", {"FDAS_CORRELATE_SCALAR": "1"}), ("v1", {"FDAS_CORRELATE_V1": "1"}),
-                      ("v0", {"FDAS_CORRELATE_V0": "1"})):
-        os.environ.update(env)
+    for name, opts in (("packed", {}), ("scalar", {fdas.FDAS_OPT_TUNE_SCALAR: 1}), ("one_chunk", {fdas.FDAS_OPT_TUNE_T_CHUNKS: 1}),
+                       ("five_chunks", {fdas.FDAS_OPT_TUNE_T_CHUNKS: 5})):
+        for k, v in opts.items():
+            fdas.fdas_plan_set_option(plan.handle, k, v)
         try:
             d_P = plan.correlate(d_S, True)[0]                        # keep the buffer alive while it is copied
             planes[name] = d_P.np().copy()
         finally:
-            for k in env:
-                os.environ.pop(k)
-    assert np.array_equal(planes["packed"], planes["scalar"])
-    for other in ("v1", "v0"):
-        assert np.max(np.abs(planes[other] - planes["packed"])) <= 2e-5 * planes["packed"].max()
+            for k in opts:
+                fdas.fdas_plan_set_option(plan.handle, k, 0)
+    for other in ("scalar", "one_chunk", "five_chunks"):
+        assert np.array_equal(planes["packed"], planes[other]), other
     thr = oracle.thresholds(16, 1e-3)
     lists = []
-    for sectors in ("1", "16", "7"):
-        os.environ["FDAS_HS_SECTORS"] = sectors
+    for opts in ({fdas.FDAS_OPT_TUNE_HS_SECTORS: 1}, {}, {fdas.FDAS_OPT_TUNE_HS_SECTORS: 7},
+                 {fdas.FDAS_OPT_TUNE_HS_ROWS: 8}, {fdas.FDAS_OPT_TUNE_HS_VARIANT: 1}):
+        for k, v in opts.items():
+            fdas.fdas_plan_set_option(plan.handle, k, v)
         try:
             c, n = plan.harmsum(E.to_dev(planes["packed"][0]), 16, thr, 1 << 16)
         finally:
-            os.environ.pop("FDAS_HS_SECTORS")
+            for k in opts:
+                fdas.fdas_plan_set_option(plan.handle, k, 0)
         lists.append(sorted((int(r["nharm"]), int(r["zi"]), int(r["col"]), float(r["power"])) for r in c))
-    assert lists[0] == lists[1] == lists[2] and len(lists[0]) > 0
+    assert all(l == lists[0] for l in lists) and len(lists[0]) > 0
     plan.close()
+
+
+def test_plane_offset_by_four_bytes(emu):
+    """include/fdas.h promises that fdas_candidates and fdas_harmsum accept a plane that is only 4-byte aligned
+    (k_candidates once took its 16-byte loads from the row offset alone)."""
+    N = 1 << 12
+    plan = emu.Plan(N, 4.0, 2.0, 16, 256, quad_points=64)
+    n_z, n_cols = plan.info.n_z, plan.info.n_cols
+    rng = np.random.default_rng(5)
+    P = rng.exponential(1.0, size=(n_z, n_cols)).astype(np.float32)
+    buf = E.DevBuf(n_z * n_cols + 1, np.float32)
+    buf.np()[1:] = P.ravel()
+
+    class Shifted:
+        def data_ptr(self):
+            return buf.ptr + 4
+
+    c, n = plan.candidates(Shifted(), 6.0, 1 << 14)
+    assert n == int((P > 6.0).sum()) and cset(c) == cset(oracle.candidates(P.astype(np.float64), 6.0))
+    thr = oracle.thresholds(16, 1e-3)
+    c, n = plan.harmsum(Shifted(), 16, thr, 1 << 16)
+    thr32 = thr.astype(np.float32)
+    cand_ok(c, oracle.harmsum(P.astype(np.float64), 16, thr, bin0=1), lambda h: float(thr32[int(h).bit_length() - 1]))
+    plan.close()
+
+
+def test_b200_geometry(monkeypatch):
+    """The persistent harmonic-sum grid and the batched fused-threshold grid at the REAL device geometry
+    (148 SMs x the occupancy ptxas gives: 2 CTAs of 128 threads for k_harmsum<5,2,2>), not the 3 x 2 pretend
+    device of the other tests: the item arithmetic (sector -> item ranges, items per CTA <= 1 for most CTAs)."""
+    monkeypatch.setenv("EMU_SMS", "148")
+    monkeypatch.setenv("EMU_CTAS_PER_SM", "2")
+    for align in ("end", "start"):
+        monkeypatch.setenv("EMU_ALIGN", align)
+        N = 1 << 16
+        plan = E.Plan(N, 16.0, 2.0, 16, 256, quad_points=64)
+        rng = np.random.default_rng(11)
+        P = rng.exponential(1.0, size=(plan.info.n_z, plan.info.n_cols)).astype(np.float32)
+        P[3, 20000] = 60.0
+        thr = oracle.thresholds(16, 1e-4)
+        c, n = plan.harmsum(E.to_dev(P), 16, thr, 1 << 16)
+        thr32 = thr.astype(np.float32)
+        cand_ok(c, oracle.harmsum(P.astype(np.float64), 16, thr, bin0=1), lambda h: float(thr32[int(h).bit_length() - 1]))
+        plan.close()
+        small = synth.small_config(1 << 13, 4.0, 2.0, 64, 2048, n_dm=64, n_sig=1, index=35, amp=0.3)   # config-3 shape: 64 DMs
+        xs = np.stack([small.series(d) for d in range(64)])
+        plan = E.Plan(1 << 13, 4.0, 2.0, 64, 2048, max_batch=64, quad_points=512)
+        d_S, _ = plan.spectrum(xs)
+        _, d_c, d_n = plan.correlate(d_S, False, 12.0, 1 << 10)
+        T = oracle.templates(4.0, 2.0, 64)
+        for d in (0, 17, 63):
+            S, _ = oracle.spectrum(xs[d])
+            cand_ok(d_c.np()[d, :int(d_n.np()[d])], oracle.candidates(oracle.correlate_direct(S, T), 12.0), lambda h: 12.0)
+        plan.close()
 
 
 def test_fused_batch(emu):
