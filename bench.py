@@ -24,7 +24,32 @@ sys.path.insert(0, ROOT)
 
 METRIC = "DM trials/s (2^23 samples, 85 z; spectrum + f-fdot plane + 16-harmonic sum)"
 UNIT = "DM trials/s"
-FP32_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12      # 148 SMs x 128 FP32 lanes x 2 (FMA) x 1.965 GHz
+FP32_LANES_PER_SM = 128                                 # Blackwell guide: 4 sub-partitions x 32 FP32 lanes
+
+
+def fp32_peak_tflops(n_sms=148, sm_mhz=1965.0):
+    """Plain-ALU FP32 peak: SMs x 128 lanes x 2 flop (FMA) x clock.  Defaults are the B200's
+    148 SMs and clocks.max.sm; run_ours() passes the SM count the device reports and, separately, the clock
+    sampled under load."""
+    return n_sms * FP32_LANES_PER_SM * 2 * sm_mhz * 1e6 / 1e12
+
+
+FP32_PEAK_TFLOPS = fp32_peak_tflops()
+
+
+def committed_traffic(kernel_substr):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the kernel whose name contains
+    `kernel_substr`, from the committed ncu summary profiles/ncu_dram_bytes.csv (kernel,read,write); None if no
+    capture has been committed (bench.py never runs under a profiler)."""
+    path = os.path.join(ROOT, "profiles", "ncu_dram_bytes.csv")
+    try:
+        for line in open(path):
+            f = [c.strip() for c in line.split(",")]
+            if len(f) >= 3 and kernel_substr in f[0] and f[1].replace(".", "").isdigit():
+                return float(f[1]) + float(f[2])
+    except OSError:
+        pass
+    return None
 
 
 def workload_flops(info):
@@ -245,6 +270,9 @@ def run_ours(args):
     if world > 1:
         dist.barrier()
     fdas.lib()
+    n_sms = torch.cuda.get_device_properties(local).multi_processor_count
+    global FP32_PEAK_TFLOPS
+    FP32_PEAK_TFLOPS = fp32_peak_tflops(n_sms)
 
     cfg = synth.config(2)
     n_rot = 4                                   # distinct resident series rotated per step: 134 MB > 126 MB L2
@@ -389,10 +417,11 @@ def run_ours(args):
     dom = max(kernels, key=lambda n: kernels[n]["ms"])          # the kernel with the largest share of the step
     kd = kernels[dom]
     roofline = {"kernel": dom + " (" + kd["kernels"] + ")", "bound": kd["bound"], "achieved": kd["achieved"],
-                "peak": kd["peak"], "unit": kd["unit"], "frac": kd["frac"], "traffic": None,
+                "peak": kd["peak"], "unit": kd["unit"], "frac": kd["frac"],
+                "traffic": committed_traffic({"spectrum": "k_spec", "correlate": "k_correlate", "harmsum": "k_harmsum"}[dom]),
                 "ms_per_launch": kd["ms"], "share_of_step": kd["ms"] / (spec_ms + corr_ms + hs_ms),
                 "peak_source": hbm_src if kd["bound"] == "hbm" else
-                "derived: 148 SM x 128 FP32 lanes x 2 x 1.965 GHz (DESIGN.md section 6)",
+                "derived: %d SMs (queried) x 128 FP32 lanes x 2 x 1.965 GHz clocks.max.sm (DESIGN.md section 6)" % n_sms,
                 "per_unit": "bytes: the plane read once (4 n_t n_bins)" if dom == "harmsum" else
                 "flops: SURVEY 8(d) convention, bench.py::workload_flops" if dom == "correlate" else "bytes: series + spectrum"}
     # north_star's FFT-correlation roofline for spectrum + correlate: the slower of flops at FP32 peak and bytes at HBM peak
@@ -414,8 +443,9 @@ def run_ours(args):
         "stage_ms": {"spectrum": spec_ms, "correlate": corr_ms, "harmsum": hs_ms},
         "stage_ms_median": dict(zip(("spectrum", "correlate", "harmsum"), (float(v) for v in np.median(stage_all, axis=0)))),
         "stage_ms_min": dict(zip(("spectrum", "correlate", "harmsum"), (float(v) for v in stage_all.min(axis=0)))),
-        "fp32_peak": {"nominal_tflops": FP32_PEAK_TFLOPS, "measured_ffma_tflops": fp32_measured,
-                      "measured_ffma2_tflops": fp32_packed},
+        "fp32_peak": {"nominal_tflops": FP32_PEAK_TFLOPS, "n_sms": n_sms, "measured_ffma_tflops": fp32_measured,
+                      "measured_ffma2_tflops": fp32_packed,
+                      "at_sampled_clock_tflops": fp32_peak_tflops(n_sms, clocks["sm_mhz"]) if clocks and clocks.get("sm_mhz") else None},
         "fft_correlation_roofline": {"ms_at_roofline": t_roof_ms, "ms_measured": spec_ms + corr_ms,
                                      "frac": t_roof_ms / (spec_ms + corr_ms),
                                      "dm_trials_per_s_without_harmsum": world * 1e3 / (spec_ms + corr_ms)},
@@ -456,6 +486,12 @@ def main():
                     help="time spectrum + correlate against the number of templates (PAPER.md Fig. 2) instead")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.gpus > 1 and "RANK" not in os.environ and args.impl == "ours" and not (args.ab or args.sweep_templates):
+        # not under torchrun: start one rank per GPU ourselves (the driver's own launch line does the same)
+        port = 29500 + os.getpid() % 2000
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+        sys.exit(subprocess.call(cmd))
     if args.ab:
         run_ab(args)
     elif args.sweep_templates:

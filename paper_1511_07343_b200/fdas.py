@@ -88,6 +88,33 @@ def _dptr(t):
     return C.c_void_p(t.data_ptr()) if t is not None else None
 
 
+def _require(t, name, numel, dtypes, device=None, allow_none=False):
+    """A device buffer handed to the C ABI: the library cannot know sizes or types, so a wrong tensor would
+    become an out-of-bounds access on the GPU.  Raise here instead (torch tensors only; anything else that
+    offers data_ptr() -- a test double -- is the caller's responsibility)."""
+    if t is None:
+        if allow_none:
+            return
+        raise ValueError("%s is required" % name)
+    if not isinstance(t, torch.Tensor):
+        return
+    if not t.is_cuda:
+        raise ValueError("%s must be a CUDA tensor (got %s)" % (name, t.device))
+    if device is not None and t.device != device:
+        raise ValueError("%s is on %s, the plan on %s" % (name, t.device, device))
+    if t.dtype not in dtypes:
+        raise ValueError("%s has dtype %s, expected one of %s" % (name, t.dtype, dtypes))
+    if not t.is_contiguous():
+        raise ValueError("%s must be contiguous" % name)
+    if t.numel() < numel:
+        raise ValueError("%s has %d elements, the call needs %d" % (name, t.numel(), numel))
+
+
+_F32 = (torch.float32,)
+_I32 = (torch.int32, torch.uint32) if hasattr(torch, "uint32") else (torch.int32,)
+_U8 = (torch.uint8,)
+
+
 def _stream(stream=None):
     s = stream if stream is not None else torch.cuda.current_stream()
     return C.c_void_p(s.cuda_stream)
@@ -127,12 +154,22 @@ def fdas_get_templates(plan) -> np.ndarray:
 
 
 def fdas_spectrum(plan, d_series, n_batch, d_spectrum, d_meanpow, d_workspace, stream=None):
+    info = fdas_plan_info(plan)
+    _require(d_series, "d_series", n_batch * info.n_samples, _F32)
+    _require(d_spectrum, "d_spectrum", n_batch * info.n_bins * 2, _F32)
+    _require(d_meanpow, "d_meanpow", n_batch, _F32, allow_none=True)
+    _require(d_workspace, "d_workspace", info.workspace_bytes, _U8)
     _check(lib().fdas_spectrum(plan, _dptr(d_series), int(n_batch), _dptr(d_spectrum), _dptr(d_meanpow),
                                _dptr(d_workspace), _stream(stream)), "fdas_spectrum")
 
 
 def fdas_correlate(plan, d_spectrum, n_batch, d_plane, threshold, d_cands, d_counts, capacity,
                    d_workspace=None, stream=None):
+    info = fdas_plan_info(plan)
+    _require(d_spectrum, "d_spectrum", n_batch * info.n_bins * 2, _F32)
+    _require(d_plane, "d_plane", n_batch * info.n_z * info.n_cols, _F32, allow_none=True)
+    _require(d_cands, "d_cands", n_batch * int(capacity) * 3, _I32, allow_none=True)
+    _require(d_counts, "d_counts", n_batch, _I32, allow_none=d_cands is None)
     _check(lib().fdas_correlate(plan, _dptr(d_spectrum), int(n_batch), _dptr(d_plane), float(threshold),
                                 _dptr(d_cands), _dptr(d_counts), int(capacity), _dptr(d_workspace),
                                 _stream(stream)), "fdas_correlate")
@@ -140,16 +177,29 @@ def fdas_correlate(plan, d_spectrum, n_batch, d_plane, threshold, d_cands, d_cou
 
 def fdas_harmsum(plan, d_plane, max_harm, thresholds, d_cands, d_count, capacity, stream=None):
     thr = np.ascontiguousarray(thresholds, dtype=np.float32)
+    info = fdas_plan_info(plan)
+    if thr.size < int(max_harm).bit_length():
+        raise ValueError("fdas_harmsum needs log2(max_harm)+1 thresholds")
+    _require(d_plane, "d_plane", info.n_z * info.n_cols, _F32)
+    _require(d_cands, "d_cands", int(capacity) * 3, _I32)
+    _require(d_count, "d_count", 1, _I32)
     _check(lib().fdas_harmsum(plan, _dptr(d_plane), int(max_harm), thr.ctypes.data_as(C.c_void_p),
                               _dptr(d_cands), _dptr(d_count), int(capacity), _stream(stream)), "fdas_harmsum")
 
 
 def fdas_candidates(plan, d_plane, threshold, d_cands, d_count, capacity, stream=None):
+    info = fdas_plan_info(plan)
+    _require(d_plane, "d_plane", info.n_z * info.n_cols, _F32)
+    _require(d_cands, "d_cands", int(capacity) * 3, _I32)
+    _require(d_count, "d_count", 1, _I32)
     _check(lib().fdas_candidates(plan, _dptr(d_plane), float(threshold), _dptr(d_cands), _dptr(d_count),
                                  int(capacity), _stream(stream)), "fdas_candidates")
 
 
 def fdas_resample(plan, d_series, beta, d_out, stream=None):
+    info = fdas_plan_info(plan)
+    _require(d_series, "d_series", info.n_samples, _F32)
+    _require(d_out, "d_out", info.n_samples, _F32)
     _check(lib().fdas_resample(plan, _dptr(d_series), float(beta), _dptr(d_out), _stream(stream)), "fdas_resample")
 
 
@@ -242,7 +292,11 @@ class Plan:
 
     # calls
     def spectrum(self, d_series, d_spectrum=None, d_meanpow=None, stream=None):
+        if d_series.dim() not in (1, 2) or d_series.shape[-1] != self.info.n_samples:
+            raise ValueError("d_series must be float32[n_samples] or [n_batch, n_samples], got %s" % (tuple(d_series.shape),))
         n_batch = d_series.shape[0] if d_series.dim() == 2 else 1
+        if n_batch > self.max_batch:
+            raise ValueError("n_batch %d exceeds the plan's MAX_BATCH %d (sizes the workspace)" % (n_batch, self.max_batch))
         if d_spectrum is None:
             d_spectrum = self.empty_spectrum(n_batch)
         if d_meanpow is None:
@@ -251,6 +305,8 @@ class Plan:
         return d_spectrum, d_meanpow
 
     def correlate(self, d_spectrum, d_plane=None, threshold=0.0, cands=None, capacity=0, stream=None):
+        if d_spectrum.dim() != 3 or tuple(d_spectrum.shape[1:]) != (self.info.n_bins, 2):
+            raise ValueError("d_spectrum must be float32[n_batch, n_bins, 2], got %s" % (tuple(d_spectrum.shape),))
         n_batch = d_spectrum.shape[0]
         d_c, d_n = cands if cands is not None else (None, None)
         fdas_correlate(self.handle, d_spectrum, n_batch, d_plane, threshold, d_c, d_n, capacity, None, stream)

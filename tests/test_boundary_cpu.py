@@ -104,6 +104,54 @@ def test_state_and_argument_errors_without_gpu(fdas):
     fdas.fdas_plan_destroy(h)
 
 
+def test_binding_refuses_wrong_tensors_before_calling_the_library(fdas):
+    """the C ABI cannot know buffer sizes, so the Python mirrors check device, dtype,
+    contiguity and element count and raise instead of launching on a wrong buffer."""
+    import torch
+    h = fdas.fdas_plan_create(1 << 12, 4, 2, 16, 256)
+    info = fdas.fdas_plan_info(h)
+    cpu_series = torch.zeros(1 << 12)
+    with pytest.raises(ValueError, match="CUDA tensor"):
+        fdas.fdas_spectrum(h, cpu_series, 1, cpu_series, None, cpu_series)
+    with pytest.raises(ValueError, match="CUDA tensor"):
+        fdas.fdas_correlate(h, torch.zeros((1, info.n_bins, 2)), 1, None, 0.0, None, None, 0)
+    with pytest.raises(ValueError, match="thresholds"):
+        fdas.fdas_harmsum(h, cpu_series, 16, np.ones(2), cpu_series, cpu_series, 4)
+    # the size / dtype / layout rules themselves (a meta tensor stands in for a CUDA one: no GPU here)
+    class FakeCuda(torch.Tensor):
+        is_cuda = True
+    def fake(*shape, dtype=torch.float32):
+        return torch.zeros(shape, dtype=dtype).as_subclass(FakeCuda)
+    with pytest.raises(ValueError, match="elements"):
+        fdas._require(fake(10), "d_plane", 11, fdas._F32)
+    with pytest.raises(ValueError, match="dtype"):
+        fdas._require(fake(10, dtype=torch.float64), "d_plane", 10, fdas._F32)
+    with pytest.raises(ValueError, match="contiguous"):
+        fdas._require(fake(10, 2)[:, 0], "d_plane", 10, fdas._F32)
+    fdas._require(fake(10), "d_plane", 10, fdas._F32)
+    fdas._require(None, "d_meanpow", 1, fdas._F32, allow_none=True)
+    with pytest.raises(ValueError, match="required"):
+        fdas._require(None, "d_plane", 1, fdas._F32)
+    fdas.fdas_plan_destroy(h)
+
+
+def test_tuning_keys_and_size_limit(fdas):
+    lib = fdas.lib()
+    h = fdas.fdas_plan_create(1 << 12, 4, 2, 16, 256)
+    for key, bad in ((fdas.FDAS_OPT_TUNE_SCALAR, 2), (fdas.FDAS_OPT_TUNE_T_CHUNKS, -1), (fdas.FDAS_OPT_TUNE_HS_SECTORS, 65),
+                     (fdas.FDAS_OPT_TUNE_HS_ROWS, 9), (fdas.FDAS_OPT_TUNE_HS_VARIANT, 2)):
+        assert lib.fdas_plan_set_option(h, key, bad) == fdas.FDAS_E_INVALID
+        assert lib.fdas_plan_set_option(h, key, 1) == fdas.FDAS_OK
+        assert lib.fdas_plan_set_option(h, key, 0) == fdas.FDAS_OK
+    fdas.fdas_plan_destroy(h)
+    # include/fdas.h: n_samples <= 2^25
+    hh = C.c_void_p()
+    assert lib.fdas_plan_create(C.byref(hh), 1 << 25, 2.0, 2.0, 256, 2048) == fdas.FDAS_OK
+    fdas.fdas_plan_destroy(hh)
+    assert lib.fdas_plan_create(C.byref(hh), 1 << 26, 2.0, 2.0, 256, 2048) == fdas.FDAS_E_INVALID
+    assert "2^25" in open(os.path.join(ROOT, "include", "fdas.h")).read()
+
+
 def test_thresholds_host_logic(fdas, golden):
     for H, T in golden("thresholds.txt"):
         assert fdas.fdas_threshold(int(H), 1e-6) == pytest.approx(T, abs=2e-9)
