@@ -57,6 +57,8 @@ extern "C" {
 #define FDAS_OPT_TUNE_HS_SECTORS 103  /* angular sectors of the harmonic-sum tile order, 1..64 (default 16) */
 #define FDAS_OPT_TUNE_HS_ROWS    104  /* warps per CTA of the harmonic-sum kernel, 1..8 (default 4) */
 #define FDAS_OPT_TUNE_HS_VARIANT 105  /* 1: 128-column harmonic-sum tiles (default 64) */
+#define FDAS_OPT_TUNE_SPEC_GENERIC 106 /* 1: the generic two-pass spectrum kernels at every length (default: the
+                                        * TMA-staged multi-pass transform from 2^13 samples on) */
 
 typedef struct fdas_plan fdas_plan;
 
@@ -107,6 +109,13 @@ int fdas_plan_info(const fdas_plan* plan, fdas_info* out);
  * (PAPER.md:49 step 5 "complex multiply - scale").  Allocates the bank (device memory
  * owned by the plan), enqueues on `stream`, and synchronises that stream once. */
 int fdas_build_templates(fdas_plan* plan, void* stream);
+
+/* Device status word of the plan, *out = 0 if all is well.  Bit 0 (FDAS_STATUS_COPY_TIMEOUT): a kernel gave up
+ * waiting for an asynchronous (TMA) copy -- its waits are bounded so that a mistake shows up here and not as
+ * a hung GPU; the results of that call are then undefined.  Synchronous (a 4-byte device-to-host copy): call it
+ * after synchronising the stream, not in the hot loop. */
+#define FDAS_STATUS_COPY_TIMEOUT 1u
+int fdas_plan_status(const fdas_plan* plan, uint32_t* out);
 
 /* Test hook: copy the fp32 taps to host, h_re_im[(t*m + j)*2 + {0,1}] = {Re, Im} T_t[j].
  * Synchronous. FDAS_E_STATE before build. */

@@ -8,7 +8,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libfdas.so")
-SOURCES = ["fdas_api.cu", "fdas_host.cu", "fdas_templates.cu", "fdas_spectrum.cu", "fdas_correlate.cu", "fdas_harmsum.cu", "fdas_peak.cu", "fdas_resample.cu"]
+SOURCES = ["fdas_api.cu", "fdas_host.cu", "fdas_templates.cu", "fdas_spectrum.cu", "fdas_spectrum_tma.cu", "fdas_tma.cu", "fdas_correlate.cu", "fdas_harmsum.cu", "fdas_peak.cu", "fdas_resample.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]
 

@@ -35,8 +35,12 @@ static void derive_sizes(fdas_plan* p)
     int c2 = 4096 / p->R2; if (c2 < 1) c2 = 1; if (c2 > p->R1 / 2) c2 = p->R1 / 2; if (c2 < 1) c2 = 1;
     p->C1 = c1; p->C2 = c2;
     p->n_part = p->R2 / p->C1;
+    fdas_spectrum_tma_plan(p);
+    // partial sums: the generic kernels use n_part per series, the TMA-staged passes M/4096 and one scale per series
+    size_t parts = (size_t)p->n_part;
+    if (p->sp_npass && (size_t)(p->M / 4096) > parts) parts = (size_t)(p->M / 4096);
     p->ws_inter_bytes = align_up((size_t)p->max_batch * p->M * sizeof(float2), 256);
-    p->ws_part_bytes = align_up((size_t)p->max_batch * p->n_part * 3 * sizeof(double), 256);
+    p->ws_part_bytes = align_up((size_t)p->max_batch * (parts * 3 * sizeof(double) + sizeof(float)), 256);
     p->workspace_bytes = p->ws_inter_bytes + p->ws_part_bytes;
 }
 
@@ -91,6 +95,7 @@ extern "C" int fdas_plan_set_option(fdas_plan* p, int32_t key, int64_t value)
     case FDAS_OPT_TUNE_HS_SECTORS: if (value < 0 || value > 64) return FDAS_E_INVALID; p->tune_hs_sectors = (int32_t)value; return FDAS_OK;
     case FDAS_OPT_TUNE_HS_ROWS:    if (value < 0 || value > 8) return FDAS_E_INVALID; p->tune_hs_rows = (int32_t)value; return FDAS_OK;
     case FDAS_OPT_TUNE_HS_VARIANT: if (value < 0 || value > 1) return FDAS_E_INVALID; p->tune_hs_variant = (int32_t)value; return FDAS_OK;
+    case FDAS_OPT_TUNE_SPEC_GENERIC: if (value < 0 || value > 1) return FDAS_E_INVALID; p->tune_spec_generic = (int32_t)value; return FDAS_OK;
     default: break;
     }
     if (p->built) return FDAS_E_STATE;
@@ -132,10 +137,23 @@ extern "C" int fdas_build_templates(fdas_plan* p, void* stream)
     if (!p->d_taps && cudaMalloc(&p->d_taps, (size_t)p->n_t * p->m * sizeof(float2)) != cudaSuccess) { p->d_taps = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
     if (!p->d_W && cudaMalloc(&p->d_W, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { p->d_W = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
     if (!p->d_Wr && cudaMalloc(&p->d_Wr, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { p->d_Wr = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
+    if (!p->d_status) {
+        if (cudaMalloc(&p->d_status, sizeof(uint32_t)) != cudaSuccess) { p->d_status = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
+        FDAS_CUDA(cudaMemsetAsync(p->d_status, 0, sizeof(uint32_t), st));
+    }
     int rc = fdas_launch_templates(p, st);
     if (rc) return rc;
     FDAS_CUDA(cudaStreamSynchronize(st));
     p->built = 1;
+    return FDAS_OK;
+}
+
+extern "C" int fdas_plan_status(const fdas_plan* p, uint32_t* out)
+{
+    if (!p || !out) return FDAS_E_INVALID;
+    *out = 0;
+    if (!p->d_status) return FDAS_OK;
+    FDAS_CUDA(cudaMemcpy(out, p->d_status, sizeof(uint32_t), cudaMemcpyDeviceToHost));
     return FDAS_OK;
 }
 
@@ -153,8 +171,8 @@ extern "C" int fdas_spectrum(fdas_plan* p, const float* d_series, int32_t n_batc
     if (!p || !d_series || !d_spectrum || n_batch < 1 || n_batch > p->max_batch) return FDAS_E_INVALID;
     if (misaligned(d_series, 8) || misaligned(d_spectrum, 8) || misaligned(d_meanpow, 4)) return FDAS_E_INVALID;
     if (!d_workspace || ((uintptr_t)d_workspace & 255)) return FDAS_E_WORKSPACE;
-    return fdas_launch_spectrum(p, d_series, n_batch, reinterpret_cast<float2*>(d_spectrum), d_meanpow,
-                                d_workspace, (cudaStream_t)stream);
+    return fdas_run_spectrum(p, d_series, n_batch, reinterpret_cast<float2*>(d_spectrum), d_meanpow, d_workspace,
+                             (cudaStream_t)stream);
 }
 
 extern "C" int fdas_correlate(fdas_plan* p, const float* d_spectrum, int32_t n_batch, float* d_plane,

@@ -12,10 +12,13 @@ struct fdas_plan {
     int32_t max_batch, quad_points;
     int32_t built;
     // tuning keys (FDAS_OPT_TUNE_*; 0 = default), read by the launchers
-    int32_t tune_scalar, tune_t_chunks, tune_hs_sectors, tune_hs_rows, tune_hs_variant;
+    int32_t tune_scalar, tune_t_chunks, tune_hs_sectors, tune_hs_rows, tune_hs_variant, tune_spec_generic;
     // big FFT split of the packed half-length transform: M = n_samples/2 = R1*R2
     int32_t M, R1, R2, C1, C2, n_part;
     size_t  ws_inter_bytes, ws_part_bytes, workspace_bytes;
+    // TMA-staged multi-pass spectrum (fdas_spectrum_tma.cu): M = 2^(la+lb+lc), 0 passes = series too short for it
+    int32_t sp_npass, sp_la, sp_lb, sp_lc;
+    uint32_t* d_status;                // device status word (bit 0: an mbarrier wait timed out), allocated with the bank
     // template bank (device, owned)
     float2* d_taps;   // [n_t][m]  conj R_z(d_j), fp32
     float2* d_W;      // [n_t][L]  FFT_L(index-reversed taps)/L, natural order
@@ -48,6 +51,18 @@ int fdas_launch_templates(fdas_plan* p, cudaStream_t st);
 int fdas_permute_templates(fdas_plan* p, cudaStream_t st);
 int fdas_launch_spectrum(fdas_plan* p, const float* d_series, int n_batch, float2* d_spec,
                          float* d_meanpow, void* d_ws, cudaStream_t st);
+void fdas_spectrum_tma_plan(fdas_plan* p);
+int fdas_launch_spectrum_tma(fdas_plan* p, const float* d_series, int n_batch, float2* d_spec,
+                             float* d_meanpow, void* d_ws, cudaStream_t st);
+// series of 2^13 samples and more take the TMA-staged multi-pass transform (tensor maps need 16-byte bases)
+inline int fdas_run_spectrum(fdas_plan* p, const float* d_series, int n_batch, float2* d_spec, float* d_meanpow, void* d_ws,
+                             cudaStream_t st)
+{
+    const bool aligned = ((reinterpret_cast<uintptr_t>(d_series) | reinterpret_cast<uintptr_t>(d_spec)) & 15) == 0;
+    if (p->sp_npass && !p->tune_spec_generic && aligned)
+        return fdas_launch_spectrum_tma(p, d_series, n_batch, d_spec, d_meanpow, d_ws, st);
+    return fdas_launch_spectrum(p, d_series, n_batch, d_spec, d_meanpow, d_ws, st);
+}
 int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float* d_plane, float thr,
                           fdas_cand* d_cands, uint32_t* d_counts, uint32_t cap, cudaStream_t st);
 int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const float* h_thr,

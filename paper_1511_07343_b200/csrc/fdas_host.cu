@@ -104,7 +104,7 @@ extern "C" int fdas_search_host(fdas_plan* p, const float* h_series, int32_t n_b
         const int b0 = c * cb, nb = chunk_nb(c);
         if (c + 1 < n_chunk) { rc = enqueue_h2d(c + 1); if (rc) return rc; }
         FDAS_CUDA(cudaStreamWaitEvent(st, p->ev_in[c & 1], 0));
-        rc = fdas_launch_spectrum(p, a.series[c & 1], nb, reinterpret_cast<float2*>(a.spec), nullptr, a.ws, st);
+        rc = fdas_run_spectrum(p, a.series[c & 1], nb, reinterpret_cast<float2*>(a.spec), nullptr, a.ws, st);
         if (rc) return rc;
         FDAS_CUDA(cudaEventRecord(p->ev_free[c & 1], st));
         if (fused) {
@@ -161,6 +161,7 @@ extern "C" int fdas_plan_destroy(fdas_plan* p)
     if (p->d_taps) cudaFree(p->d_taps);
     if (p->d_W) cudaFree(p->d_W);
     if (p->d_Wr) cudaFree(p->d_Wr);
+    if (p->d_status) cudaFree(p->d_status);
     if (p->arena) cudaFree(p->arena);
     if (p->pinned_counts) cudaFreeHost(p->pinned_counts);
     if (p->pipe_ready) {

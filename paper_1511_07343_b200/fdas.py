@@ -18,13 +18,14 @@ LIB_PATH = os.path.join(_HERE, "libfdas.so")
 
 FDAS_OK, FDAS_E_INVALID, FDAS_E_STATE, FDAS_E_WORKSPACE, FDAS_E_CUDA, FDAS_E_NOMEM = 0, -1, -2, -3, -4, -5
 FDAS_OPT_INTERBIN, FDAS_OPT_MAX_BATCH, FDAS_OPT_QUAD_POINTS = 1, 2, 3
-FDAS_OPT_TUNE_SCALAR, FDAS_OPT_TUNE_T_CHUNKS, FDAS_OPT_TUNE_HS_SECTORS, FDAS_OPT_TUNE_HS_ROWS, FDAS_OPT_TUNE_HS_VARIANT = 101, 102, 103, 104, 105
+FDAS_OPT_TUNE_SCALAR, FDAS_OPT_TUNE_T_CHUNKS, FDAS_OPT_TUNE_HS_SECTORS, FDAS_OPT_TUNE_HS_ROWS, FDAS_OPT_TUNE_HS_VARIANT, FDAS_OPT_TUNE_SPEC_GENERIC = 101, 102, 103, 104, 105, 106
+FDAS_STATUS_COPY_TIMEOUT = 1
 
 CAND_DTYPE = np.dtype([("col", "<i4"), ("zi", "<i2"), ("nharm", "<i2"), ("power", "<f4")])
 assert CAND_DTYPE.itemsize == 12
 
 EXPORTS = ["fdas_set_device", "fdas_plan_create", "fdas_plan_set_option", "fdas_plan_info",
-           "fdas_build_templates", "fdas_get_templates", "fdas_spectrum", "fdas_correlate",
+           "fdas_build_templates", "fdas_plan_status", "fdas_get_templates", "fdas_spectrum", "fdas_correlate",
            "fdas_harmsum", "fdas_candidates", "fdas_resample", "fdas_search_host", "fdas_threshold", "fdas_measure_fp32_tflops",
            "fdas_plan_destroy", "fdas_strerror"]
 
@@ -59,6 +60,7 @@ def lib():
         L.fdas_plan_set_option.argtypes = [vp, i32, i64]
         L.fdas_plan_info.argtypes = [vp, C.POINTER(FdasInfo)]
         L.fdas_build_templates.argtypes = [vp, vp]
+        L.fdas_plan_status.argtypes = [vp, C.POINTER(u32)]
         L.fdas_get_templates.argtypes = [vp, vp]
         L.fdas_spectrum.argtypes = [vp, vp, i32, vp, vp, vp, vp]
         L.fdas_correlate.argtypes = [vp, vp, i32, vp, f32, vp, vp, u32, vp, vp]
@@ -144,6 +146,12 @@ def fdas_plan_info(plan) -> FdasInfo:
 
 def fdas_build_templates(plan, stream=None):
     _check(lib().fdas_build_templates(plan, _stream(stream)), "fdas_build_templates")
+
+
+def fdas_plan_status(plan) -> int:
+    out = C.c_uint32()
+    _check(lib().fdas_plan_status(plan, C.byref(out)), "fdas_plan_status")
+    return out.value
 
 
 def fdas_get_templates(plan) -> np.ndarray:
@@ -267,6 +275,11 @@ class Plan:
         self.max_batch = max_batch
         fdas_build_templates(self.handle)
         self.workspace = torch.empty(self.info.workspace_bytes, dtype=torch.uint8, device=self.device)
+
+    def status(self):
+        """Device status word (0 = fine); synchronises the device first."""
+        torch.cuda.synchronize(self.device)
+        return fdas_plan_status(self.handle)
 
     def close(self):
         if self.handle is not None:

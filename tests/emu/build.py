@@ -18,7 +18,7 @@ def _stale() -> bool:
         return True
     t = os.path.getmtime(LIB)
     deps = [os.path.join(CSRC, f) for f in os.listdir(CSRC)]
-    deps += [os.path.join(HERE, f) for f in ("cuda_runtime.h", "emu_rt.cpp", "prep.py", "build.py")]
+    deps += [os.path.join(HERE, f) for f in ("cuda_runtime.h", "emu_tma.h", "emu_rt.cpp", "selftest_tma.cpp", "prep.py", "build.py")]
     deps.append(os.path.join(ROOT, "include", "fdas.h"))
     return any(os.path.getmtime(d) > t for d in deps)
 
@@ -36,12 +36,15 @@ def build(force: bool = False) -> str:
     shutil.copy(os.path.join(ROOT, "include", "fdas.h"), os.path.join(OUT, "include", "fdas.h"))
     units = []
     for f in sorted(os.listdir(CSRC)):
+        if f == "fdas_tma.cuh":                          # inline PTX: emu_tma.h stands in for it (prep.py)
+            continue
         text = prep.rewrite(open(os.path.join(CSRC, f)).read())
         dst = os.path.join(src_dir, f[:-3] + ".cpp" if f.endswith(".cu") else f)
         open(dst, "w").write(text)
         if f.endswith(".cu"):
             units.append(dst)
     units.append(os.path.join(HERE, "emu_rt.cpp"))
+    units.append(os.path.join(HERE, "selftest_tma.cpp"))
     procs, objs = [], []
     for u in units:
         o = os.path.join(OUT, os.path.basename(u)[:-4] + ".o")

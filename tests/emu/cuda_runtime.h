@@ -106,6 +106,7 @@ template <class T> static inline T __ldcs(const T* p)
     return *p;
 }
 static inline unsigned atomicAdd(unsigned* p, unsigned v) { return __atomic_fetch_add(p, v, __ATOMIC_RELAXED); }
+static inline unsigned atomicOr(unsigned* p, unsigned v) { return __atomic_fetch_or(p, v, __ATOMIC_RELAXED); }
 
 static inline void sincospif(float x, float* s, float* c)
 {

@@ -1,5 +1,6 @@
 // Host emulation runtime: guard-paged "device" memory + coroutine CTA scheduler (test infrastructure, tests/emu/README.md).
 #include "cuda_runtime.h"
+#include "emu_tma.h"
 #include <signal.h>
 #include <sys/mman.h>
 #include <ucontext.h>
@@ -91,7 +92,7 @@ __attribute__((constructor)) static void install()
 }
 
 // ------------------------------------------------------------------ CTA scheduler
-enum { ST_RUN = 0, ST_BLOCK_BAR = 1, ST_WARP_BAR = 2, ST_DONE = 3 };
+enum { ST_RUN = 0, ST_BLOCK_BAR = 1, ST_WARP_BAR = 2, ST_DONE = 3, ST_SPIN = 4 };   // ST_SPIN: a failed mbarrier wait, to be retried
 #if defined(__x86_64__)
 // Minimal user-level context switch (callee-saved registers + stack pointer): swapcontext makes a
 // signal-mask system call per switch, which dominates the run time of barrier-heavy kernels.
@@ -123,11 +124,16 @@ static void ctx_make(Ctx* c, char* stack, size_t size, void (*fn)(), Ctx* link)
     makecontext(&c->uc, fn, 0);
 }
 #endif
-struct Fiber { Ctx ctx; char* stack; int state; uint3 tid; unsigned n_ballot; };
+// a box of a tensor map (or a contiguous run) to be copied when its mbarrier is waited on / its store group is waited for
+struct EmuCopy { bool tensor; void* smem; const void* gmem; uint32_t bytes; CUtensorMap map; int c[3]; };
+struct EmuMbar { uint32_t init; int64_t pending; int64_t tx; uint32_t phase; std::vector<EmuCopy> loads; };
+struct Fiber { Ctx ctx; char* stack; int state; uint3 tid; unsigned n_ballot;
+               std::vector<EmuCopy> store_open, store_committed; };
 struct Worker {
     std::vector<Fiber> fibers;
     std::vector<unsigned> ballot;            // [warp][2]: alternating accumulators of __ballot_sync
     std::vector<unsigned> shfl;              // [thread]: the value each lane offers to __shfl_sync
+    std::map<uintptr_t, EmuMbar> mbars;      // the CTA's mbarrier objects, by shared-memory address
     Ctx sched;
     int cur;
     const std::function<void()>* body;
@@ -141,6 +147,11 @@ static void tramp()
     Worker* w = t_w;
     (*w->body)();
     w = t_w;
+    if (!w->fibers[w->cur].store_open.empty() || !w->fibers[w->cur].store_committed.empty()) {
+        fprintf(stderr, "EMU: %s block (%u,%u,%u) thread %d exits with bulk stores that were not committed and waited for\n",
+                t_kernel, blockIdx.x, blockIdx.y, blockIdx.z, w->cur);
+        abort();
+    }
     w->fibers[w->cur].state = ST_DONE;
     ctx_switch(&w->fibers[w->cur].ctx, &w->sched);
     abort();                                     // a finished fibre is never resumed
@@ -192,6 +203,168 @@ int emu_env_int(const char* name, int dflt)
     return v > 0 ? v : dflt;
 }
 
+
+// ------------------------------------------------------------------ mbarrier + bulk / tensor-map copies (emu_tma.h)
+struct EmuMap { uint64_t magic; const char* base; int rank; int elem; uint64_t dims[3]; uint64_t strides[2]; uint32_t box[3]; };
+static const uint64_t EMU_MAP_MAGIC = 0x544d41454d55ull;
+static void tma_fail(const char* what)
+{
+    fprintf(stderr, "EMU: %s in %s block (%u,%u,%u) thread (%u,%u)\n", what, t_kernel, blockIdx.x, blockIdx.y, blockIdx.z,
+            threadIdx.x, threadIdx.y);
+    abort();
+}
+static CUresult emu_cuTensorMapEncodeTiled(CUtensorMap* out, CUtensorMapDataType type, cuuint32_t rank, void* base,
+                                           const cuuint64_t* dims, const cuuint64_t* strides, const cuuint32_t* box,
+                                           const cuuint32_t* estr, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion,
+                                           CUtensorMapFloatOOBfill)
+{
+    if (!out || rank < 1 || rank > 3 || ((uintptr_t)base & 15)) return CUDA_ERROR_INVALID_VALUE;
+    EmuMap m; memset(&m, 0, sizeof(m));
+    m.magic = EMU_MAP_MAGIC; m.base = (const char*)base; m.rank = (int)rank; m.elem = (int)type;
+    for (cuuint32_t i = 0; i < rank; i++) {
+        if (dims[i] == 0 || box[i] == 0 || box[i] > 256 || estr[i] != 1) return CUDA_ERROR_INVALID_VALUE;
+        m.dims[i] = dims[i]; m.box[i] = box[i];
+    }
+    if (((uint64_t)box[0] * m.elem) & 15) return CUDA_ERROR_INVALID_VALUE;        // inner box extent: a multiple of 16 bytes
+    for (cuuint32_t i = 0; i + 1 < rank; i++) {
+        if (strides[i] & 15) return CUDA_ERROR_INVALID_VALUE;
+        m.strides[i] = strides[i];
+    }
+    static_assert(sizeof(EmuMap) <= sizeof(CUtensorMap), "EmuMap must fit");
+    memcpy(out, &m, sizeof(m));
+    return CUDA_SUCCESS;
+}
+cudaError_t cudaGetDriverEntryPoint(const char* symbol, void** fn, unsigned long long, cudaDriverEntryPointQueryResult* q)
+{
+    const bool ok = !strcmp(symbol, "cuTensorMapEncodeTiled");
+    *fn = ok ? (void*)emu_cuTensorMapEncodeTiled : nullptr;
+    if (q) *q = ok ? cudaDriverEntryPointSuccess : cudaDriverEntryPointSymbolNotFound;
+    return cudaSuccess;
+}
+static uint64_t box_bytes(const EmuMap& m)
+{
+    uint64_t n = m.elem;
+    for (int i = 0; i < m.rank; i++) n *= m.box[i];
+    return n;
+}
+// move one box between shared memory (dense, innermost first) and the tensor; outside the tensor: zeros / skipped
+static void run_copy(const EmuCopy& c, bool to_smem)
+{
+    if (!c.tensor) {
+        if (to_smem) memcpy(c.smem, c.gmem, c.bytes); else memcpy(const_cast<void*>(c.gmem), c.smem, c.bytes);
+        return;
+    }
+    EmuMap m; memcpy(&m, &c.map, sizeof(m));
+    char* sp = (char*)c.smem;
+    const uint32_t b1 = m.rank > 1 ? m.box[1] : 1, b2 = m.rank > 2 ? m.box[2] : 1;
+    for (uint32_t i2 = 0; i2 < b2; i2++)
+        for (uint32_t i1 = 0; i1 < b1; i1++)
+            for (uint32_t i0 = 0; i0 < m.box[0]; i0++, sp += m.elem) {
+                const long long x0 = (long long)c.c[0] + i0, x1 = (long long)c.c[1] + i1, x2 = (long long)c.c[2] + i2;
+                const bool in = x0 >= 0 && x0 < (long long)m.dims[0] && (m.rank < 2 || (x1 >= 0 && x1 < (long long)m.dims[1])) &&
+                                (m.rank < 3 || (x2 >= 0 && x2 < (long long)m.dims[2]));
+                char* gp = const_cast<char*>(m.base) + x0 * m.elem + (m.rank > 1 ? x1 * (long long)m.strides[0] : 0) +
+                           (m.rank > 2 ? x2 * (long long)m.strides[1] : 0);
+                if (to_smem) { if (in) memcpy(sp, gp, m.elem); else memset(sp, 0, m.elem); }
+                else if (in) memcpy(gp, sp, m.elem);
+            }
+}
+static EmuMbar& mbar_of(uint64_t* bar, bool must_exist = true)
+{
+    if ((uintptr_t)bar & 7) tma_fail("misaligned mbarrier");
+    auto& tab = t_w->mbars;
+    auto it = tab.find((uintptr_t)bar);
+    if (it == tab.end()) {
+        if (must_exist) tma_fail("use of an mbarrier that was not initialised in this CTA");
+        it = tab.emplace((uintptr_t)bar, EmuMbar{0, 0, 0, 0, {}}).first;
+    }
+    return it->second;
+}
+static void mbar_check(EmuMbar& b)
+{
+    if (b.pending < 0) tma_fail("more arrivals on an mbarrier than its count");
+    if (b.pending == 0 && b.tx == 0) { b.phase++; b.pending = b.init; }
+}
+void mbar_init(uint64_t* bar, uint32_t arrivals)
+{
+    EmuMbar& b = mbar_of(bar, false);
+    b.init = arrivals; b.pending = arrivals; b.tx = 0; b.phase = 0; b.loads.clear();
+}
+void mbar_expect_tx(uint64_t* bar, uint32_t bytes) { EmuMbar& b = mbar_of(bar); b.tx += bytes; b.pending--; mbar_check(b); }
+void mbar_arrive(uint64_t* bar) { EmuMbar& b = mbar_of(bar); b.pending--; mbar_check(b); }
+bool mbar_try_wait(uint64_t* bar, uint32_t parity)
+{
+    return (mbar_of(bar).phase & 1u) != (parity & 1u);
+}
+// The copy engines: the bytes of every issued load land at the END of a scheduling round, i.e. after every runnable
+// thread has had its turn -- not at issue -- so that a read of the destination that is not ordered after the
+// mbarrier wait sees poison.  Returns whether anything moved.
+static bool land_loads(Worker* w)
+{
+    bool any = false;
+    for (auto& kv : w->mbars) {
+        EmuMbar& b = kv.second;
+        std::vector<EmuCopy> q;
+        q.swap(b.loads);
+        for (const EmuCopy& c : q) {
+            run_copy(c, true);
+            b.tx -= c.bytes;
+            mbar_check(b);
+            any = true;
+        }
+    }
+    return any;
+}
+bool mbar_wait(uint64_t* bar, uint32_t parity, uint32_t*)
+{
+    for (;;) {
+        if (mbar_try_wait(bar, parity)) return true;
+        yield_with(ST_SPIN);
+        t_w->fibers[t_w->cur].state = ST_RUN;
+    }
+}
+static void queue_load(EmuCopy c, uint64_t* bar, size_t smem_align)
+{
+    if ((uintptr_t)c.smem & (smem_align - 1)) tma_fail("bulk copy: shared-memory address not aligned");
+    if (c.bytes == 0 || (c.bytes & 15)) tma_fail("bulk copy: size is not a positive multiple of 16 bytes");
+    memset(c.smem, 0xFF, c.bytes);                          // until the wait, the destination holds poison
+    mbar_of(bar).loads.push_back(c);
+}
+void tma_load_1d(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar)
+{
+    if ((uintptr_t)gmem_src & 15) tma_fail("bulk copy: global address not 16-byte aligned");
+    emu_check_ptr(gmem_src, 1, "bulk copy source");
+    queue_load(EmuCopy{false, smem_dst, gmem_src, bytes, {}, {0, 0, 0}}, bar, 16);
+}
+static EmuCopy tensor_copy(void* smem, const CUtensorMap* map, int rank, int c0, int c1, int c2)
+{
+    EmuMap m; memcpy(&m, map, sizeof(m));
+    if (m.magic != EMU_MAP_MAGIC) tma_fail("tensor copy through a map that was never encoded");
+    if (m.rank != rank) tma_fail("tensor copy: rank of the instruction differs from the map's");
+    EmuCopy c{true, smem, nullptr, (uint32_t)box_bytes(m), *map, {c0, c1, c2}};
+    return c;
+}
+void tma_load_2d(void* smem_dst, const CUtensorMap* map, int c0, int c1, uint64_t* bar) { queue_load(tensor_copy(smem_dst, map, 2, c0, c1, 0), bar, 128); }
+void tma_load_3d(void* smem_dst, const CUtensorMap* map, int c0, int c1, int c2, uint64_t* bar) { queue_load(tensor_copy(smem_dst, map, 3, c0, c1, c2), bar, 128); }
+void tma_store_3d(const CUtensorMap* map, const void* smem_src, int c0, int c1, int c2)
+{
+    if ((uintptr_t)smem_src & 127) tma_fail("tensor store: shared-memory address not 128-byte aligned");
+    t_w->fibers[t_w->cur].store_open.push_back(tensor_copy(const_cast<void*>(smem_src), map, 3, c0, c1, c2));
+}
+void tma_store_commit()
+{
+    Fiber& f = t_w->fibers[t_w->cur];
+    for (auto& c : f.store_open) f.store_committed.push_back(c);
+    f.store_open.clear();
+}
+void tma_store_wait_read()
+{
+    Fiber& f = t_w->fibers[t_w->cur];
+    for (const EmuCopy& c : f.store_committed) run_copy(c, false);        // shared memory is read NOW
+    f.store_committed.clear();
+}
+void tma_store_wait_all() { tma_store_wait_read(); }
+
 static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward, 1 reversed, >= 2 pseudo-random (seed)
 {
     const bool rev = order == 1;
@@ -208,10 +381,12 @@ static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward
         ctx_make(&f.ctx, f.stack, STACK, tramp, &w->sched);
         f.state = ST_RUN;
         f.n_ballot = 0;
+        f.store_open.clear(); f.store_committed.clear();
         f.tid = uint3{(unsigned)i % block.x, ((unsigned)i / block.x) % block.y, (unsigned)i / (block.x * block.y)};
     }
     w->ballot.assign(2 * ((nt + 31) / 32), 0u);
     w->shfl.assign(32 * ((nt + 31) / 32), 0u);
+    w->mbars.clear();
     int done = 0;
     while (done < nt) {
         bool progress = false;
@@ -226,13 +401,14 @@ static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward
         for (int q = 0; q < nt; q++) {
             int i = order >= 2 ? perm[q] : (rev ? nt - 1 - q : q);
             Fiber& f = w->fibers[i];
-            if (f.state != ST_RUN) continue;
+            if (f.state != ST_RUN && f.state != ST_SPIN) continue;
             w->cur = i;
             threadIdx = f.tid;
             ctx_switch(&w->sched, &f.ctx);
-            progress = true;
+            if (f.state != ST_SPIN) progress = true;     // a fibre that only re-tried a failed mbarrier wait made no progress
             if (f.state == ST_DONE) done++;
         }
+        if (land_loads(w)) progress = true;
         // release warp barriers
         for (int w0 = 0; w0 < nt; w0 += 32) {
             int at = 0, live = 0;
@@ -257,7 +433,10 @@ static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward
             abort();
         }
         if (!progress) {
-            fprintf(stderr, "EMU: deadlock in %s block (%u,%u,%u)\n", t_kernel, blockIdx.x, blockIdx.y, blockIdx.z);
+            int spin = 0;
+            for (int i = 0; i < nt; i++) spin += w->fibers[i].state == ST_SPIN;
+            fprintf(stderr, "EMU: deadlock in %s block (%u,%u,%u)%s\n", t_kernel, blockIdx.x, blockIdx.y, blockIdx.z,
+                    spin ? ": an mbarrier wait can never be satisfied (arrivals or announced bytes do not match)" : "");
             abort();
         }
     }

@@ -35,7 +35,11 @@ def split_top(a):
     return out
 
 def rewrite(s):
-    s = re.sub(r"extern\s+__shared__\s+(\w+)\s+(\w+)\[\];", r"\1* \2 = (\1*)emu_dyn_smem();", s)
+    # the asynchronous-copy wrappers (inline PTX) are replaced by the emulator's model of them
+    s = s.replace('#include "fdas_tma.cuh"', '#include "emu_tma.h"')
+    # the asynchronous-copy wrappers (inline PTX) are replaced by the emulator's model of them
+    s = s.replace('#include "fdas_tma.cuh"', '#include "emu_tma.h"')
+    s = re.sub(r"extern\s+__shared__\s+(?:__align__\(\d+\)\s+)?(\w+)\s+(\w+)\[\];", r"\1* \2 = (\1*)emu_dyn_smem();", s)
     while True:
         i = s.find("<<<")
         if i < 0: break

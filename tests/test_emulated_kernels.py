@@ -52,7 +52,9 @@ def cand_ok(c_gpu, c_ref, thr_of):
         assert abs(pw[k] - thr_of(k[0])) <= 1e-4 * thr_of(k[0]), k
 
 
-@pytest.mark.parametrize("log2n", [9, 10, 13, 16])
+# 2^9, 2^10, 2^12: the generic kernels; 2^13 .. 2^17: two TMA-staged passes (factors 64x64 .. 256x256);
+# 2^18, 2^19: three passes (32x32x128, 32x32x256)
+@pytest.mark.parametrize("log2n", [9, 10, 12, 13, 14, 15, 16, 17, 18, 19])
 def test_spectrum(emu, log2n):
     N = 1 << log2n
     x = synth.make_series(N, 4242 + log2n, [synth.Signal(0.2, N / 8 + 0.3, 2.0, 0.5)])
@@ -63,6 +65,38 @@ def test_spectrum(emu, log2n):
     S_ref, mu = oracle.spectrum(x)
     assert float(d_mu.np()[0]) == pytest.approx(mu, rel=2e-6)
     assert np.max(np.abs(S[:, 0] + 1j * S[:, 1] - S_ref)) <= 3e-6 * np.max(np.abs(S_ref)) + 2e-5
+    assert fdas.fdas_plan_status(plan.handle) == 0
+    plan.close()
+
+
+def test_spectrum_paths_agree_and_fall_back(emu):
+    """The TMA-staged passes and the generic kernels give the same spectrum to rounding (each within 1e-6 rms of
+    the oracle); a series that is only 8-byte aligned (tensor maps need 16) silently takes the generic kernels."""
+    N = 1 << 15
+    xs = np.stack([synth.make_series(N, 500 + b) * (1.0 + 0.5 * b) for b in range(2)])
+    S = {}
+    for generic in (0, 1):
+        plan = emu.Plan(N, 4.0, 2.0, 16, 256, max_batch=2, quad_points=64)
+        fdas.fdas_plan_set_option(plan.handle, fdas.FDAS_OPT_TUNE_SPEC_GENERIC, generic)
+        d_S, d_mu = plan.spectrum(xs)
+        S[generic] = d_S.np().copy()
+        for b in range(2):
+            S_ref, mu = oracle.spectrum(xs[b])
+            z = S[generic][b][:, 0] + 1j * S[generic][b][:, 1]
+            assert np.sqrt(np.mean(np.abs(z - S_ref) ** 2)) < 1e-6 and float(d_mu.np()[b]) == pytest.approx(mu, rel=2e-6)
+        plan.close()
+    assert np.max(np.abs(S[0] - S[1])) < 5e-6
+    plan = emu.Plan(N, 4.0, 2.0, 16, 256, quad_points=64)
+    buf = E.DevBuf(N + 2, np.float32)
+    buf.np()[2:] = xs[0]
+
+    class Shifted:
+        def data_ptr(self):
+            return buf.ptr + 8
+
+    d_S = E.DevBuf((1, N // 2, 2), np.float32)
+    fdas.fdas_spectrum(plan.handle, Shifted(), 1, d_S, None, plan.workspace)
+    assert np.max(np.abs(d_S.np()[0] - S[1][0])) == 0.0                  # bit for bit the generic kernels' result
     plan.close()
 
 
@@ -79,8 +113,8 @@ def test_all_zero_series(emu):
     plan.close()
 
 
-def test_spectrum_batched(emu):
-    N = 1 << 12
+@pytest.mark.parametrize("N", [1 << 12, 1 << 13])
+def test_spectrum_batched(emu, N):
     xs = np.stack([synth.make_series(N, 900 + b) * (1.0 + b) for b in range(3)])
     plan = emu.Plan(N, 4.0, 2.0, 16, 256, max_batch=3, quad_points=64)
     d_S, d_mu = plan.spectrum(xs)
@@ -345,3 +379,30 @@ else:
     assert short.returncode == 99 and "illegal access" in short.stderr and "k_candidates" in short.stderr, short.stderr[-500:]
     mis = subprocess.run([sys.executable, "-c", prog, "misaligned"], capture_output=True, text=True, timeout=300)
     assert mis.returncode == 0, mis.stderr[-500:]
+
+
+def test_the_emulator_models_the_asynchronous_copies():
+    """The emulator's model of mbarriers and TMA copies (tests/emu/emu_tma.h), tried on small kernels that use them
+    correctly and incorrectly (tests/emu/selftest_tma.cpp): a read before the wait sees poison, a byte count that
+    does not match is a reported deadlock, a store that is not waited for, a misaligned box buffer and a source
+    buffer reused too early are all caught.  Without this the TMA-staged kernels' emulator runs would prove little."""
+    import subprocess
+    prog = r'''
+import ctypes, sys
+sys.path.insert(0, %r)
+from emu import build
+L = ctypes.CDLL(build.build())
+sys.exit(10 + L.emu_selftest_tma(int(sys.argv[1])))
+''' % os.path.dirname(os.path.abspath(__file__))
+    env = dict(os.environ, EMU_ORDER="fwd", EMU_THREADS="1")
+    def run(mode):
+        return subprocess.run([sys.executable, "-c", prog, str(mode)], capture_output=True, text=True, timeout=300, env=env)
+    assert run(0).returncode == 10                                      # correct use: output right
+    assert run(1).returncode == 11                                      # early read saw NaN poison
+    r = run(2)
+    assert r.returncode not in (10, 11) and "mbarrier wait can never be satisfied" in r.stderr, r.stderr[-300:]
+    r = run(3)
+    assert r.returncode not in (10, 11) and "not committed and waited for" in r.stderr, r.stderr[-300:]
+    r = run(4)
+    assert r.returncode not in (10, 11) and "not aligned" in r.stderr, r.stderr[-300:]
+    assert run(5).returncode == 11                                      # buffer reused too early: output corrupted

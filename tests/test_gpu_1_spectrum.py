@@ -25,6 +25,28 @@ def test_spectrum_matches_oracle(fdas, log2n):
     assert float(d_mu[0]) == pytest.approx(mu, rel=2e-6)
     scale = np.sqrt(np.mean(np.abs(S_ref) ** 2))         # = 1
     assert np.max(np.abs(S_gpu - S_ref)) <= 3e-6 * np.max(np.abs(S_ref)) + 2e-5 * scale
+    assert plan.status() == 0                            # no asynchronous copy timed out
+
+
+def test_spectrum_paths_agree(fdas):
+    """The TMA-staged multi-pass transform (default from 2^13 samples) against the generic two-pass kernels
+    (tuning key): same spectrum to rounding, both within 1e-6 rms of the oracle, two and three passes."""
+    for log2n in (14, 18):
+        N = 1 << log2n
+        xs = np.stack([synth.make_series(N, 500 + b) * (1.0 + 0.5 * b) for b in range(2)])
+        S = {}
+        for generic in (0, 1):
+            plan = fdas.Plan(N, 4.0, 2.0, 16, 256, max_batch=2)
+            fdas.fdas_plan_set_option(plan.handle, fdas.FDAS_OPT_TUNE_SPEC_GENERIC, generic)
+            d_S, d_mu = plan.spectrum(torch.from_numpy(xs).cuda())
+            S[generic] = d_S.cpu().numpy()
+            assert plan.status() == 0
+            for b in range(2):
+                S_ref, mu = oracle.spectrum(xs[b])
+                z = S[generic][b][:, 0] + 1j * S[generic][b][:, 1]
+                assert np.sqrt(np.mean(np.abs(z - S_ref) ** 2)) < 1e-6
+                assert float(d_mu[b]) == pytest.approx(mu, rel=2e-6)
+        assert np.max(np.abs(S[0] - S[1])) < 5e-6
 
 
 def test_spectrum_batched(fdas):
