@@ -44,10 +44,10 @@ __device__ __forceinline__ void dft_fwd(float2* v)
     float2 w[R];
 #pragma unroll
     for (int j = 0; j < R; j++) w[brev(j, LR)] = v[j];
-    if constexpr (LR >= 1) dit_const_stage<R, -1, 1>(w);
-    if constexpr (LR >= 2) dit_const_stage<R, -1, 2>(w);
-    if constexpr (LR >= 3) dit_const_stage<R, -1, 3>(w);
-    if constexpr (LR >= 4) dit_const_stage<R, -1, 4>(w);
+    if constexpr (LR >= 1) dit_const_stage<R, -1, 1, true>(w);
+    if constexpr (LR >= 2) dit_const_stage<R, -1, 2, true>(w);
+    if constexpr (LR >= 3) dit_const_stage<R, -1, 3, true>(w);
+    if constexpr (LR >= 4) dit_const_stage<R, -1, 4, true>(w);
 #pragma unroll
     for (int j = 0; j < R; j++) v[j] = w[j];
 }
@@ -117,21 +117,33 @@ k_spec_cols(const __grid_constant__ CUtensorMap in, const __grid_constant__ CUte
     __syncthreads();
 #pragma unroll
     for (int i = 0; i < 16; i++) v[i] = tin[(16 * t + i) * T + c];
+    // pass twiddle W_D^{x y}, y = y0 + ymul k, k = r + 16 q:  W^{x (y0 + ymul r)} (W^{16 x ymul})^q -- one sincospif
+    // per group and one for the step, whose powers come from products of depth <= 4 (a few 1e-8 of extra error);
+    // every exponent is reduced mod D as an integer first and is exact in fp32 (D <= 2^24)
     const int col = c0 + c;
     const unsigned x = (unsigned)col >> a.xs, y0 = (unsigned)(a.y0_mul * outer), dmask = (1u << a.logD) - 1u;
-    const float dinv = 1.0f / (float)(1u << a.logD);
+    const float dinv = 2.0f / (float)(1u << a.logD);
+    float2 st[P];                                     // st[q] = step^q
+    st[0] = make_float2(1.0f, 0.0f);
+    {
+        const unsigned e = (16u * x * (unsigned)a.ymul) & dmask;
+        float sn, cs;
+        sincospif((float)e * dinv, &sn, &cs);
+        st[1] = make_float2(cs, -sn);
+#pragma unroll
+        for (int q = 2; q < P; q++) st[q] = cmul(st[q >> 1], st[q - (q >> 1)]);
+    }
 #pragma unroll
     for (int g = 0; g < G; g++) {
         dft_fwd<LP>(v + g * P);
         const int r = G * t + g;
+        const unsigned e = (x * (y0 + (unsigned)(a.ymul * r))) & dmask;
+        float sn, cs;
+        sincospif((float)e * dinv, &sn, &cs);
+        const float2 base = make_float2(cs, -sn);
 #pragma unroll
-        for (int q = 0; q < P; q++) {
-            const int k = r + 16 * q;
-            const unsigned e = (x * (y0 + (unsigned)(a.ymul * k))) & dmask;      // < 2^24: exact in fp32
-            float sn, cs;
-            sincospif(2.0f * (float)e * dinv, &sn, &cs);
-            tout[k * T + c] = cmul(v[g * P + q], make_float2(cs, -sn));
-        }
+        for (int q = 0; q < P; q++)
+            tout[(r + 16 * q) * T + c] = cmul(v[g * P + q], q == 0 ? base : cmul(base, st[q]));
     }
     fence_proxy_async();
     if constexpr (ACC_POWER) {                        // fixed-order tree over the CTA (deterministic)
