@@ -150,6 +150,124 @@ __device__ __forceinline__ void harmsum_tile(const float* __restrict__ plane, fd
 #undef HS_V
 }
 
+// ---- interior tiles: the row body specialised on its move pattern --------------------------------------------
+// Which streams move to a new source row depends only on |zeta| mod 16 and on the side of zeta = 0 (the
+// condition above involves t mod H, H | 16): 32 patterns.  harmsum_tile evaluates the pattern at run time
+// (ballot + R2P) and ptxas if-converts every stream into ~8 predicated instructions that issue whether or not
+// the stream moved (129 instructions per row and 2 cells).  Here the pattern is a TEMPLATE argument: a row
+// jumps (one warp-uniform switch) to the body compiled for its pattern, which contains exactly the pointer
+// bumps and loads of the streams that move -- 8 of 15 on average -- into the registers that carry the values
+// from row to row; no predicates, no index arithmetic (one 64-bit pointer per stream, bumped by the row
+// stride), no ballot.  With 4 cells per lane the stage sums are 30 FADD2 and 20 compares per row.
+__host__ __device__ constexpr unsigned hs_moved_mask(int r16, bool positive, int nst)
+{
+    unsigned m = 1u;                                                   // slot 0 (P itself) always moves
+    for (int st = 1; st < nst; st++) {
+        const int H = 1 << st;
+        for (int h = 1; h < H; h += 2) {
+            const int fr = (r16 * h + (H >> 1)) & (H - 1);
+            if (positive ? fr < h : fr + h >= H) m |= 1u << ((H >> 1) + (h >> 1));
+        }
+    }
+    return m;
+}
+
+template <int NST, int HS_CPT, unsigned MASK>
+__device__ __forceinline__ void hs_fetch_row(const float* (&ptr)[1 << (NST - 1)], float2 (&v)[HS_CPT / 2][1 << (NST - 1)],
+                                             long long stride)
+{
+#define HS_V(j, i) (((j) & 1) ? v[(j) >> 1][i].y : v[(j) >> 1][i].x)
+    ptr[0] += stride;
+#pragma unroll
+    for (int j = 0; j < HS_CPT; j++) HS_V(j, 0) = __ldcs(ptr[0] + 32 * j);
+#pragma unroll
+    for (int st = 1; st < NST; st++) {
+        const int H = 1 << st;
+#pragma unroll
+        for (int h = 1; h < H; h += 2) {
+            const int slot = (H >> 1) + (h >> 1);
+            if (MASK & (1u << slot)) {                                 // compile time
+                ptr[slot] += stride;
+                const int dk = (32 * h) >> st;                         // exact: 32 h / H
+#pragma unroll
+                for (int j = 0; j < HS_CPT; j++) HS_V(j, slot) = __ldg(ptr[slot] + dk * j);
+            }
+        }
+    }
+#undef HS_V
+}
+
+#define HS_CASE(R, POS) case R: hs_fetch_row<NST, HS_CPT, hs_moved_mask(R, POS, NST)>(ptr, v, stride); break;
+#define HS_CASES(POS) HS_CASE(0, POS) HS_CASE(1, POS) HS_CASE(2, POS) HS_CASE(3, POS) HS_CASE(4, POS) HS_CASE(5, POS) HS_CASE(6, POS) \
+    HS_CASE(7, POS) HS_CASE(8, POS) HS_CASE(9, POS) HS_CASE(10, POS) HS_CASE(11, POS) HS_CASE(12, POS) HS_CASE(13, POS)               \
+    HS_CASE(14, POS) HS_CASE(15, POS)
+
+// Interior tile (every k_h >= bin0, every column < n_cols): rows [zi_lo, zi_hi) of 32 HS_CPT columns, one warp.
+template <int NST, int HS_CPT>
+__device__ __forceinline__ void harmsum_tile_fast(const float* __restrict__ plane, fdas_cand* __restrict__ cands,
+                                                  uint32_t* __restrict__ count, uint32_t cap, const HarmThr& thr,
+                                                  int n_cols, int n_z, int bin0, int tile, int zi_lo, int zi_hi)
+{
+    constexpr int HS_COLS = 32 * HS_CPT;
+    constexpr int HMAX = 1 << (NST - 1);
+    static_assert(HS_CPT % 2 == 0, "cells are summed in pairs (packed f32x2 adds)");
+    const int lane = threadIdx.x;
+    const int col0 = tile * HS_COLS + lane;
+    const int zc = (n_z - 1) / 2;
+    const int k = bin0 + col0;
+    if (zi_lo >= zi_hi) return;                                        // the whole warp
+    const long long stride = n_cols;
+    // one pointer per stream, ONE ROW BEFORE its first source row: the first row moves every stream
+    const float* ptr[HMAX];
+    {
+        const int zeta0 = zi_lo - zc, az0 = abs(zeta0), sg0 = zeta0 < 0 ? -1 : 1;
+        ptr[0] = plane + ((long long)(zi_lo - 1) * n_cols + col0);
+#pragma unroll
+        for (int st = 1; st < NST; st++) {
+            const int H = 1 << st;
+#pragma unroll
+            for (int h = 1; h < H; h += 2) {
+                const int slot = (H >> 1) + (h >> 1);
+                const int kh = (k * h + (H >> 1)) >> st;              // k*h < 2^29 for n_samples <= 2^25
+                const int zh0 = sg0 * ((az0 * h + (H >> 1)) >> st);
+                ptr[slot] = plane + ((long long)(zc + zh0 - 1) * n_cols + (kh - bin0));
+            }
+        }
+    }
+    float2 v[HS_CPT / 2][HMAX];                                       // .x, .y = cells 2jj, 2jj+1 of the lane
+#pragma unroll 1
+    for (int zi = zi_lo; zi < zi_hi; zi++) {
+        const int zeta = zi - zc, r16 = abs(zeta) & 15;                // warp-uniform
+        if (zi == zi_lo) hs_fetch_row<NST, HS_CPT, 0xffffffffu>(ptr, v, stride);
+        else if (zeta > 0) { switch (r16) { HS_CASES(true) } }
+        else { switch (r16) { HS_CASES(false) } }
+#pragma unroll
+        for (int jj = 0; jj < HS_CPT / 2; jj++) {
+            float2 sum[NST];
+            float2 acc = v[jj][0];
+            sum[0] = acc;
+            bool any = acc.x > thr.t[0] || acc.y > thr.t[0];
+#pragma unroll
+            for (int st = 1; st < NST; st++) {
+                const int H = 1 << st;
+#pragma unroll
+                for (int i = H >> 1; i < H; i++) acc = __fadd2_rn(acc, v[jj][i]);
+                sum[st] = acc;
+                any = any || acc.x > thr.t[st] || acc.y > thr.t[st];
+            }
+            if (__any_sync(0xffffffffu, any)) {                         // rare; warp-uniform: the ballots below see all 32 lanes
+#pragma unroll
+                for (int st = 0; st < NST; st++) {
+                    push_cand_hs(cands, count, cap, sum[st].x > thr.t[st], col0 + 32 * (2 * jj), zi, 1 << st, sum[st].x);
+                    push_cand_hs(cands, count, cap, sum[st].y > thr.t[st], col0 + 32 * (2 * jj + 1), zi, 1 << st, sum[st].y);
+                }
+            }
+        }
+    }
+}
+#undef HS_CASES
+#undef HS_CASE
+
 // Tile order.  The stretch (k, zeta) -> (k h/H, zeta h/H) moves a cell along the ray through the origin of
 // the (k, zeta) plane, so the 16 cells that read one source cell all lie on that ray, at k = x H/h: with the
 // plain order (all rows of a column tile together, columns ascending) they are 1/16 ... 15/16 of the plane
@@ -211,8 +329,13 @@ k_harmsum(const float* __restrict__ plane, fdas_cand* __restrict__ cands, uint32
         if (tile >= n_tiles) continue;
         const int row_part = sec.col_warps > 1 ? 0 : (int)threadIdx.y, n_row_parts = sec.col_warps > 1 ? 1 : (int)blockDim.y;
         const bool edge = tile == 0 || tile * HS_COLS + HS_COLS > n_cols;
-        if (edge) harmsum_tile<NST, HS_CPT, true>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi, row_part, n_row_parts);
-        else harmsum_tile<NST, HS_CPT, false>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi, row_part, n_row_parts);
+        if (edge) {
+            harmsum_tile<NST, HS_CPT, true>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, zi_lo, zi_hi, row_part, n_row_parts);
+        } else {                             // interior: this warp's rows of the tile (all of them, or its part in the plain order)
+            const int rpw = (zi_hi - zi_lo + n_row_parts - 1) / n_row_parts;
+            const int r_begin = zi_lo + row_part * rpw, r_end = min(zi_hi, r_begin + rpw);
+            harmsum_tile_fast<NST, HS_CPT>(plane, cands, count, cap, thr, n_cols, n_z, bin0, tile, r_begin, r_end);
+        }
     }
 }
 
