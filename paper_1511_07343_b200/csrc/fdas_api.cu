@@ -141,6 +141,14 @@ extern "C" int fdas_build_templates(fdas_plan* p, void* stream)
         if (cudaMalloc(&p->d_status, sizeof(uint32_t)) != cudaSuccess) { p->d_status = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
         FDAS_CUDA(cudaMemsetAsync(p->d_status, 0, sizeof(uint32_t), st));
     }
+    {
+        int dev = 0, sms = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) {
+            cudaGetLastError();
+            sms = 148;
+        }
+        p->n_sms = sms > 0 ? sms : 148;
+    }
     int rc = fdas_launch_templates(p, st);
     if (rc) return rc;
     FDAS_CUDA(cudaStreamSynchronize(st));

@@ -11,6 +11,7 @@ struct fdas_plan {
     double  z_max, dz;
     int32_t max_batch, quad_points;
     int32_t built;
+    int32_t n_sms;                     // SMs of the device the bank was built on (launch geometry)
     // tuning keys (FDAS_OPT_TUNE_*; 0 = default), read by the launchers
     int32_t tune_scalar, tune_t_chunks, tune_hs_sectors, tune_hs_rows, tune_hs_variant, tune_spec_generic;
     // big FFT split of the packed half-length transform: M = n_samples/2 = R1*R2

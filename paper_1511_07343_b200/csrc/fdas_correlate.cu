@@ -268,7 +268,13 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
 {
     if (d_cands) FDAS_CUDA(cudaMemsetAsync(d_counts, 0, sizeof(uint32_t) * n_batch, st));
     if (p->L == 2048) {
-        int n_chunk = p->tune_t_chunks > 0 ? p->tune_t_chunks : (p->n_t + 28) / 29;      // ~29 templates per CTA: short tail
+        // Template chunks per segment.  A single series (2341 segments at 2^23 samples) needs ~29 templates per CTA to
+        // fill 148 SMs x 3 CTAs for many waves (short tail), at the price of one forward FFT per chunk (+3.5 %).  A batch
+        // that gives >= 20 waves by itself (configs[3]: 64 series) lets one CTA own ALL templates of its segment: the
+        // forward FFT and the twiddle set-up are done once per segment (SURVEY section 7 hard part 2).
+        const long long slots = 3LL * (p->n_sms > 0 ? p->n_sms : 148);
+        const bool one_chunk = (long long)p->n_seg * n_batch >= 20 * slots;
+        int n_chunk = p->tune_t_chunks > 0 ? p->tune_t_chunks : one_chunk ? 1 : (p->n_t + 28) / 29;
         int t_chunk = (p->n_t + n_chunk - 1) / n_chunk;
         n_chunk = (p->n_t + t_chunk - 1) / t_chunk;
         dim3 grid(p->n_seg, n_chunk, n_batch);

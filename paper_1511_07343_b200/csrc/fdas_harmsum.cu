@@ -303,7 +303,7 @@ __host__ __device__ inline double sector_boundary(int j, int S, double kc, doubl
 }
 
 template <int NST, int HS_CPT, int MINB>
-__global__ void __launch_bounds__(256, MINB)
+__global__ void __launch_bounds__(MINB >= 3 ? 128 : 256, MINB)           // MINB >= 3: at most 4 warps per CTA (the launcher sees to it)
 k_harmsum(const float* __restrict__ plane, fdas_cand* __restrict__ cands, uint32_t* __restrict__ count,
           uint32_t cap, HarmThr thr, HarmSectors sec, int n_cols, int n_z, int bin0)
 {
@@ -426,6 +426,7 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     HarmSectors sec;
 #define FDAS_HS_LAUNCH(NST, CPT, MINB)                                                              \
     do {                                                                                            \
+        if (MINB >= 3 && rows > 4) { rows = 4; block = dim3(32, rows); }   /* launch bound of that instance */ \
         sec = make_sectors(n_sec, n_sec == 1 ? 1 : rows, n_cols, p->bin0, 32 * CPT);                                       \
         int n_cta = resident_ctas(k_harmsum<NST, CPT, MINB>, 32 * rows);                            \
         if (n_cta > sec.first_item[n_sec]) n_cta = sec.first_item[n_sec];                           \
@@ -438,8 +439,8 @@ int fdas_launch_harmsum(fdas_plan* p, const float* d_plane, int max_harm, const 
     case 3: FDAS_HS_LAUNCH(3, 4, 2); break;
     case 4: FDAS_HS_LAUNCH(4, 2, 2); break;
     default:
-        if (variant == 1) FDAS_HS_LAUNCH(5, 4, 1);        // 128-column tiles, ~190 registers, ~67 instructions per cell: to be timed against the default
-        else FDAS_HS_LAUNCH(5, 2, 2);                    // 64-column tiles, 118 registers, no spills (cuobjdump: ~90 instructions per cell and row)
+        if (variant == 1) FDAS_HS_LAUNCH(5, 2, 2);        // 64-column tiles, 128 registers, 4 CTAs/SM: ~45 instructions per cell (tuning key)
+        else FDAS_HS_LAUNCH(5, 4, 3);                    // 128-column tiles, 3 CTAs of 4 warps per SM: ~33 instructions per cell (profiles/)
         break;
     }
 #undef FDAS_HS_LAUNCH
