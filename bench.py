@@ -328,6 +328,7 @@ def run_ours(args):
     fp32_measured, _ = fdas.fdas_measure_fp32_tflops()       # FFMA-chain microbenchmark (untimed region)
     fp32_packed, _ = fdas.fdas_measure_fp32_tflops(packed=True)
     n_found = int(cands[1][0])
+    assert plan.status() == 0, "an asynchronous copy timed out in the timed region (fdas_plan_status)"
 
     # BASELINE.json configs[3] (streaming batch, plane not stored, threshold fused into the segment kernel):
     # a batch of 8 resident DM trials per call, spectrum + fused correlate, reported beside the headline
@@ -401,15 +402,16 @@ def run_ours(args):
     plane_bytes = 4 * info.n_templates * info.n_bins
     corr_tf = flops / (corr_ms * 1e-3) / 1e12
     kernels = {
-        "spectrum": {"kernels": "k_spec_pass1 + k_spec_pass2", "bound": "hbm", "ms": spec_ms,
+        "spectrum": {"kernels": "k_spec_cols (pass A, pass B) + k_spec_scale + k_spec_rows (pass C): TMA-staged", "bound": "hbm", "ms": spec_ms,
                      "algorithmic_bytes": 4 * cfg.n_samples + 8 * info.n_bins,
                      "achieved": (4 * cfg.n_samples + 8 * info.n_bins) / (spec_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s"},
-        "correlate": {"kernels": "k_correlate_2048_v2", "bound": "alu", "ms": corr_ms, "algorithmic_flops": flops,
+        "correlate": {"kernels": "k_correlate_2048", "bound": "alu", "ms": corr_ms, "algorithmic_flops": flops,
                       "achieved": corr_tf, "peak": FP32_PEAK_TFLOPS, "unit": "TFLOP/s",
                       "peak_measured_ffma": fp32_measured, "frac_of_measured_ffma": corr_tf / fp32_measured,
                       "hbm_side": {"bytes": plane_bytes + 8 * info.n_bins,
                                    "achieved_gbs": (plane_bytes + 8 * info.n_bins) / (corr_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak}},
-        "harmsum": {"kernels": "k_harmsum<5,...>", "bound": "hbm", "ms": hs_ms, "algorithmic_bytes": plane_bytes,
+        "harmsum": {"kernels": "k_harmsum<5,4,3>", "bound": "hbm", "ms": hs_ms, "algorithmic_bytes": plane_bytes,
+                    "l2_to_sm_bytes_inherent": 5.84 * plane_bytes,    # sum over the 16 streams of (h/16)^2
                     "achieved": plane_bytes / (hs_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s"},
     }
     for k in kernels.values():
@@ -454,7 +456,8 @@ def run_ours(args):
                         "ms_per_dm": fused_ms, "dm_trials_per_s": world * 1e3 / fused_ms,
                         "frac_of_fft_roofline": t_roof3_ms / fused_ms, "candidates_found": fused_found},
         "candidates_found": n_found,
-        "gpu_launches": 4 * args.steps,
+        "gpu_launches": 6 * args.steps,        # 4 spectrum kernels + fused correlate + harmonic sum (+ 1 memset node)
+        "plan_status": plan.status(),
         "clocks": clocks,
         "e2e": {"value": world * 1e3 / e2e_ms, "unit": UNIT, "ms_per_step": e2e_ms,
                 "h2d_bytes_per_step": cfg.n_samples * 4, "d2h_bytes_per_step": d2h,
