@@ -95,6 +95,7 @@ extern "C" int fdas_plan_set_option(fdas_plan* p, int32_t key, int64_t value)
     case FDAS_OPT_TUNE_HS_SECTORS: if (value < 0 || value > 64) return FDAS_E_INVALID; p->tune_hs_sectors = (int32_t)value; return FDAS_OK;
     case FDAS_OPT_TUNE_HS_ROWS:    if (value < 0 || value > 8) return FDAS_E_INVALID; p->tune_hs_rows = (int32_t)value; return FDAS_OK;
     case FDAS_OPT_TUNE_HS_VARIANT: if (value < 0 || value > 1) return FDAS_E_INVALID; p->tune_hs_variant = (int32_t)value; return FDAS_OK;
+    case FDAS_OPT_TUNE_STAGE_TEMPLATES: if (value < 0 || value > 1) return FDAS_E_INVALID; p->tune_stage_templates = (int32_t)value; return FDAS_OK;
     case FDAS_OPT_TUNE_SPEC_GENERIC: if (value < 0 || value > 1) return FDAS_E_INVALID; p->tune_spec_generic = (int32_t)value; return FDAS_OK;
     default: break;
     }

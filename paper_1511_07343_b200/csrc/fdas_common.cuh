@@ -13,7 +13,7 @@ struct fdas_plan {
     int32_t built;
     int32_t n_sms;                     // SMs of the device the bank was built on (launch geometry)
     // tuning keys (FDAS_OPT_TUNE_*; 0 = default), read by the launchers
-    int32_t tune_scalar, tune_t_chunks, tune_hs_sectors, tune_hs_rows, tune_hs_variant, tune_spec_generic;
+    int32_t tune_scalar, tune_t_chunks, tune_hs_sectors, tune_hs_rows, tune_hs_variant, tune_spec_generic, tune_stage_templates;
     // big FFT split of the packed half-length transform: M = n_samples/2 = R1*R2
     int32_t M, R1, R2, C1, C2, n_part;
     size_t  ws_inter_bytes, ws_part_bytes, workspace_bytes;

@@ -5,6 +5,7 @@
 #include "fdas_common.cuh"
 #include "fdas_smemfft.cuh"
 #include "fdas_regfft.cuh"
+#include "fdas_tma.cuh"
 
 // Generic segment length (L != 2048; natural-order smem Stockham): one CTA per (segment, batch entry).
 // smem: X[L] | A[L] | B[L].
@@ -128,20 +129,36 @@ __device__ __forceinline__ void seg_pass3(const float2* buf, const float2* tw_a,
     }
 }
 
-template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK>
-__global__ void __launch_bounds__(SEG_THREADS, 3)
-k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
-                    fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
-                    int n_bins, int n_z, int m, int step, int t_chunk)
+// Shared state of the STAGED variant (k_correlate_2048_staged): NG segments ("groups" of 128 threads) per CTA take
+// every template spectrum from a two-slot ring in shared memory that ONE thread fills with 16 KB bulk copies
+// (cp.async.bulk, fdas_tma.cuh).  full[b]: the copy into slot b has landed (1 arrival + 16384 bytes);
+// empty[b]: every warp of the CTA has copied slot b into its registers (4 NG arrivals).
+struct SegStage {
+    const float4* wbuf;       // [2][8 * SEG_THREADS]
+    uint64_t* full;           // [2]
+    uint64_t* empty;          // [2]
+    uint32_t* status;
+    int group;                // 0 .. NG-1 (the named barrier of the group is 1 + group)
+    bool producer;            // thread 0 of the CTA
+};
+
+// One overlap-save segment against the templates [t_begin, t_end): the body of both kernels.  NG == 1: the
+// 128-thread CTA of k_correlate_2048 (template spectra by LDG from L2/L1, __syncthreads).  NG > 1: one group of
+// the staged kernel (template spectra from the ring, group barriers).  `tid` is the thread's index in its group.
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK, int NG>
+__device__ __forceinline__ void correlate_segment(float2* sm, const int tid, const int seg, const int bt, const int t_begin,
+                                                  const int t_end, const float2* __restrict__ spec,
+                                                  const float4* __restrict__ Wr, float* __restrict__ plane,
+                                                  fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap,
+                                                  float thr, int n_bins, int n_z, int m, int step, const SegStage& stg)
 {
     constexpr int L = 2048;
     constexpr int nset = NSET;
-    __shared__ __align__(16) float2 sm[2 * SEG_BUF];
-    const int tid = threadIdx.x;
     const int lo = tid & 15, k3A = tid >> 4;
-    const int seg = blockIdx.x, bt = blockIdx.z;
-    const int n_t = n_z * nset;
-    const int t_begin = blockIdx.y * t_chunk, t_end = min(n_t, t_begin + t_chunk);
+    auto group_barrier = [&]() {
+        if constexpr (NG == 1) __syncthreads();
+        else named_bar_sync(1 + stg.group, SEG_THREADS);
+    };
     const int c0 = seg * step;
     const float2* S = spec + (size_t)bt * n_bins;
 
@@ -164,7 +181,7 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
                 buf[p + SEG_PITCH3 * k3] = val;
             }
         }
-        __syncthreads();
+        group_barrier();
         float2 v[16];
 #pragma unroll
         for (int n2 = 0; n2 < 16; n2++) v[bitrev(n2, 4)] = buf[lo + 16 * n2 + SEG_PITCH3 * k3A];
@@ -180,7 +197,7 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
         dit_const<16, -1, PK>(v);
 #pragma unroll
         for (int k1 = 0; k1 < 16; k1++) X[k1] = v[k1];
-        __syncthreads();
+        group_barrier();
     }
 
     float2 tw2[8], tw3[2][4];
@@ -198,13 +215,24 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
 
     float4 w4[8];
     const float4* Wn = Wr + (size_t)t_begin * (8 * SEG_THREADS) + tid;      // template whose spectrum is fetched next
-    if (t_begin < t_end) {
+    if constexpr (NG == 1) {
+        if (t_begin < t_end) {
 #pragma unroll
-        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * SEG_THREADS);
+            for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * SEG_THREADS);
+        }
     }
     float* prow1 = HAS_PLANE ? pbase + (size_t)t_begin * n_cols : nullptr;  // NSET == 1: row of template t
     for (int t = t_begin; t < t_end; t++) {
         float2* buf = sm + ((t - t_begin) & 1) * SEG_BUF;
+        if constexpr (NG > 1) {                                                  // slot b = use k of the ring: parity k & 1
+            const int b = (t - t_begin) & 1, k = (t - t_begin) >> 1;
+            if (!mbar_wait(stg.full + b, k & 1, stg.status)) return;
+            const float4* ws = stg.wbuf + b * (8 * SEG_THREADS) + tid;
+#pragma unroll
+            for (int j = 0; j < 8; j++) w4[j] = ws[j * SEG_THREADS];
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(stg.empty + b);
+        }
         float2 v[16];
         if (PK) mul_first_stage16_pk(v, X, w4);                                  // X W and stage 1
         else mul_first_stage16(v, X, w4);
@@ -227,10 +255,18 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
         __syncwarp();
 #pragma unroll
         for (int t2 = 0; t2 < 16; t2++) buf[lo + 16 * t2 + SEG_PITCH3 * k3A] = v[t2];
-        if (t + 1 < t_end) Wn += 8 * SEG_THREADS;                                 // (the last iteration re-reads its own)
+        if constexpr (NG == 1) {
+            if (t + 1 < t_end) Wn += 8 * SEG_THREADS;                             // (the last iteration re-reads its own)
 #pragma unroll
-        for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * SEG_THREADS);
-        __syncthreads();
+            for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * SEG_THREADS);
+        } else if (stg.producer && t + 2 < t_end) {                               // refill this iteration's slot with template t + 2
+            const int b = (t - t_begin) & 1, k = (t - t_begin) >> 1;
+            if (!mbar_wait(stg.empty + b, k & 1, stg.status)) return;
+            mbar_expect_tx(stg.full + b, 8 * SEG_THREADS * 16);
+            tma_load_1d(const_cast<float4*>(stg.wbuf) + b * (8 * SEG_THREADS), Wr + (size_t)(t + 2) * (8 * SEG_THREADS),
+                        8 * SEG_THREADS * 16, stg.full + b);
+        }
+        group_barrier();
         const int zi = NSET == 1 ? t : (t >> 1), s = NSET == 1 ? 0 : (t & 1);
         float* prow = !HAS_PLANE ? nullptr : NSET == 1 ? prow1 : pbase + (size_t)zi * n_cols + s;
         if (HAS_PLANE && NSET == 1) prow1 += n_cols;
@@ -239,6 +275,77 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
             seg_pass3<HAS_PLANE, HAS_CANDS, NSET, NKEEP, true, PK>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
         else
             seg_pass3<HAS_PLANE, HAS_CANDS, NSET, 8, false, PK>(buf, tw3[0], tw3[1], tid, prow, nv, clist, ccount, cap, thr, col0, zi);
+    }
+}
+
+
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK>
+__global__ void __launch_bounds__(SEG_THREADS, 3)
+k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
+                    fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
+                    int n_bins, int n_z, int m, int step, int t_chunk)
+{
+    __shared__ __align__(16) float2 sm[2 * SEG_BUF];
+    const int n_t = n_z * NSET;
+    const int t_begin = blockIdx.y * t_chunk, t_end = min(n_t, t_begin + t_chunk);
+    correlate_segment<HAS_PLANE, HAS_CANDS, NSET, NKEEP, PK, 1>(sm, threadIdx.x, blockIdx.x, blockIdx.z, t_begin, t_end, spec, Wr,
+                                                                 plane, cands, counts, cap, thr, n_bins, n_z, m, step, SegStage{});
+}
+
+// STAGED variant (tuning key FDAS_OPT_TUNE_STAGE_TEMPLATES; SURVEY section 7 hard part 2, "several segments per
+// template load"): one CTA = SEG_GROUPS groups of 128 threads = SEG_GROUPS adjacent segments; every template
+// spectrum crosses L2 -> SM ONCE per CTA, as a 16 KB bulk copy (UBLKCP) into a two-slot ring, instead of once
+// per segment: 1.1 GB instead of up to 3.3 GB per DM trial at configs[2], whatever L1 does.  Groups run
+// independently between ring accesses (their own exchange buffers and named barrier).  A group whose segment
+// lies beyond the series (last CTA) only keeps the ring protocol going.
+// dynamic shared memory: ring [2][16 KB] | exchange buffers [SEG_GROUPS][2][SEG_BUF] | 4 mbarriers.
+constexpr int SEG_GROUPS = 3;
+constexpr int SEG_RING_BYTES = 2 * 8 * SEG_THREADS * 16;
+constexpr int SEG_STAGED_SMEM = SEG_RING_BYTES + SEG_GROUPS * 2 * SEG_BUF * 8 + 128;
+
+template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK>
+__global__ void __launch_bounds__(SEG_GROUPS* SEG_THREADS, 1)
+k_correlate_2048_staged(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
+                        fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
+                        int n_bins, int n_z, int m, int step, int t_chunk, int n_seg, uint32_t* status)
+{
+    extern __shared__ __align__(128) float2 dsm[];
+    float4* ring = reinterpret_cast<float4*>(dsm);
+    float2* exch = dsm + SEG_RING_BYTES / 8;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(exch + SEG_GROUPS * 2 * SEG_BUF);
+    const int group = threadIdx.x / SEG_THREADS, tid = threadIdx.x % SEG_THREADS;
+    const int n_t = n_z * NSET;
+    const int t_begin = blockIdx.y * t_chunk, t_end = min(n_t, t_begin + t_chunk);
+    SegStage stg;
+    stg.wbuf = ring; stg.full = bars; stg.empty = bars + 2; stg.status = status; stg.group = group;
+    stg.producer = threadIdx.x == 0;
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < 2; b++) {
+            mbar_init(stg.full + b, 1);
+            mbar_init(stg.empty + b, SEG_GROUPS * SEG_THREADS / 32);
+        }
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int b = 0; b < 2 && t_begin + b < t_end; b++) {
+            mbar_expect_tx(stg.full + b, 8 * SEG_THREADS * 16);
+            tma_load_1d(ring + b * (8 * SEG_THREADS), Wr + (size_t)(t_begin + b) * (8 * SEG_THREADS), 8 * SEG_THREADS * 16,
+                        stg.full + b);
+        }
+    }
+    const int seg = blockIdx.x * SEG_GROUPS + group;
+    if (seg < n_seg) {
+        correlate_segment<HAS_PLANE, HAS_CANDS, NSET, NKEEP, PK, SEG_GROUPS>(exch + group * 2 * SEG_BUF, tid, seg, blockIdx.z, t_begin,
+                                                                           t_end, spec, Wr, plane, cands, counts, cap, thr, n_bins,
+                                                                           n_z, m, step, stg);
+    } else {                                   // no segment: consume the ring so that the producer's waits complete
+        for (int t = t_begin; t < t_end; t++) {
+            const int b = (t - t_begin) & 1, k = (t - t_begin) >> 1;
+            if (!mbar_wait(stg.full + b, k & 1, status)) return;
+            __syncwarp();
+            if ((tid & 31) == 0) mbar_arrive(stg.empty + b);
+        }
     }
 }
 
@@ -285,6 +392,27 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
         else if (d_plane) k_correlate_2048<true, false, __VA_ARGS__><<<grid, SEG_THREADS, 0, st>>>(FDAS_SEG_ARGS);      \
         else k_correlate_2048<false, true, __VA_ARGS__><<<grid, SEG_THREADS, 0, st>>>(FDAS_SEG_ARGS)
         const bool scalar = p->tune_scalar != 0;                  // scalar FFMA butterflies (tuning key; bit-identical planes)
+        if (p->tune_stage_templates && !scalar) {                 // several segments per template load (see k_correlate_2048_staged)
+            dim3 sgrid((p->n_seg + SEG_GROUPS - 1) / SEG_GROUPS, n_chunk, n_batch);
+#define FDAS_STG_LAUNCH(...)                                                                                                   \
+            do {                                                                                                               \
+                FDAS_CUDA(cudaFuncSetAttribute(k_correlate_2048_staged<__VA_ARGS__>, cudaFuncAttributeMaxDynamicSharedMemorySize, \
+                                               SEG_STAGED_SMEM));                                                              \
+                k_correlate_2048_staged<__VA_ARGS__><<<sgrid, SEG_GROUPS * SEG_THREADS, SEG_STAGED_SMEM, st>>>(                \
+                    FDAS_SEG_ARGS, p->n_seg, p->d_status);                                                                     \
+            } while (0)
+#define FDAS_STG_LAUNCH_NS(NS, NK)                                                           \
+            if (d_plane && d_cands) FDAS_STG_LAUNCH(true, true, NS, NK, true);               \
+            else if (d_plane) FDAS_STG_LAUNCH(true, false, NS, NK, true);                    \
+            else FDAS_STG_LAUNCH(false, true, NS, NK, true)
+            const bool k7 = p->step == 7 * 256;
+            if (p->nset == 1) { if (k7) { FDAS_STG_LAUNCH_NS(1, 7); } else { FDAS_STG_LAUNCH_NS(1, 8); } }
+            else { if (k7) { FDAS_STG_LAUNCH_NS(2, 7); } else { FDAS_STG_LAUNCH_NS(2, 8); } }
+#undef FDAS_STG_LAUNCH_NS
+#undef FDAS_STG_LAUNCH
+            FDAS_LAUNCH_CHECK();
+            return FDAS_OK;
+        }
         const bool keep7 = p->step == 7 * 256;                    // m = 256: full segments keep t3 < 7 exactly
 #define FDAS_SEG_LAUNCH_NS(NS)                                                                   \
         if (keep7 && !scalar) { FDAS_SEG_LAUNCH(NS, 7, true); }                                  \

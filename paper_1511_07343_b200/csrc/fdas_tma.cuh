@@ -112,6 +112,12 @@ __device__ __forceinline__ void tma_prefetch_map(const CUtensorMap* map)
     asm volatile("prefetch.tensormap [%0];" ::"l"(map) : "memory");
 }
 
+// barrier `id` (1..15; 0 is __syncthreads) among `n_threads` threads of the CTA (a multiple of 32: whole warps)
+__device__ __forceinline__ void named_bar_sync(int id, int n_threads)
+{
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n_threads) : "memory");
+}
+
 // ------------------------------------------------------------------ host: tensor-map encoding
 // Tensor of 8-byte elements (a float2 / complex value is one element), rank 2 or 3, dims[0] innermost and
 // contiguous, strides_bytes[i] = byte stride of dims[i+1] (multiples of 16), box[i] <= 256 elements.

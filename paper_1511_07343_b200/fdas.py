@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libfdas.so")
 
 FDAS_OK, FDAS_E_INVALID, FDAS_E_STATE, FDAS_E_WORKSPACE, FDAS_E_CUDA, FDAS_E_NOMEM = 0, -1, -2, -3, -4, -5
 FDAS_OPT_INTERBIN, FDAS_OPT_MAX_BATCH, FDAS_OPT_QUAD_POINTS = 1, 2, 3
-FDAS_OPT_TUNE_SCALAR, FDAS_OPT_TUNE_T_CHUNKS, FDAS_OPT_TUNE_HS_SECTORS, FDAS_OPT_TUNE_HS_ROWS, FDAS_OPT_TUNE_HS_VARIANT, FDAS_OPT_TUNE_SPEC_GENERIC = 101, 102, 103, 104, 105, 106
+FDAS_OPT_TUNE_SCALAR, FDAS_OPT_TUNE_T_CHUNKS, FDAS_OPT_TUNE_HS_SECTORS, FDAS_OPT_TUNE_HS_ROWS, FDAS_OPT_TUNE_HS_VARIANT, FDAS_OPT_TUNE_SPEC_GENERIC, FDAS_OPT_TUNE_STAGE_TEMPLATES = 101, 102, 103, 104, 105, 106, 107
 FDAS_STATUS_COPY_TIMEOUT = 1
 
 CAND_DTYPE = np.dtype([("col", "<i4"), ("zi", "<i2"), ("nharm", "<i2"), ("power", "<f4")])

@@ -92,7 +92,7 @@ __attribute__((constructor)) static void install()
 }
 
 // ------------------------------------------------------------------ CTA scheduler
-enum { ST_RUN = 0, ST_BLOCK_BAR = 1, ST_WARP_BAR = 2, ST_DONE = 3, ST_SPIN = 4 };   // ST_SPIN: a failed mbarrier wait, to be retried
+enum { ST_RUN = 0, ST_BLOCK_BAR = 1, ST_WARP_BAR = 2, ST_DONE = 3, ST_SPIN = 4, ST_NAMED_BAR = 5 };   // ST_SPIN: a failed mbarrier wait, to be retried
 #if defined(__x86_64__)
 // Minimal user-level context switch (callee-saved registers + stack pointer): swapcontext makes a
 // signal-mask system call per switch, which dominates the run time of barrier-heavy kernels.
@@ -127,7 +127,7 @@ static void ctx_make(Ctx* c, char* stack, size_t size, void (*fn)(), Ctx* link)
 // a box of a tensor map (or a contiguous run) to be copied when its mbarrier is waited on / its store group is waited for
 struct EmuCopy { bool tensor; void* smem; const void* gmem; uint32_t bytes; CUtensorMap map; int c[3]; };
 struct EmuMbar { uint32_t init; int64_t pending; int64_t tx; uint32_t phase; std::vector<EmuCopy> loads; };
-struct Fiber { Ctx ctx; char* stack; int state; uint3 tid; unsigned n_ballot;
+struct Fiber { Ctx ctx; char* stack; int state; uint3 tid; unsigned n_ballot; int bar_id, bar_n;
                std::vector<EmuCopy> store_open, store_committed; };
 struct Worker {
     std::vector<Fiber> fibers;
@@ -364,6 +364,14 @@ void tma_store_wait_read()
     f.store_committed.clear();
 }
 void tma_store_wait_all() { tma_store_wait_read(); }
+// bar.sync id, n: released when n threads of the CTA wait on barrier `id` (they must agree on n)
+void named_bar_sync(int id, int n_threads)
+{
+    if (id < 1 || id > 15 || n_threads < 32 || (n_threads & 31)) tma_fail("named barrier: id not in 1..15 or thread count not whole warps");
+    Fiber& f = t_w->fibers[t_w->cur];
+    f.bar_id = id; f.bar_n = n_threads;
+    yield_with(ST_NAMED_BAR);
+}
 
 static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward, 1 reversed, >= 2 pseudo-random (seed)
 {
@@ -419,6 +427,24 @@ static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward
             if (live && at == live) {
                 for (int i = w0; i < w0 + 32 && i < nt; i++)
                     if (w->fibers[i].state == ST_WARP_BAR) w->fibers[i].state = ST_RUN;
+                progress = true;
+            }
+        }
+        for (int id = 1; id <= 15; id++) {                       // named barriers
+            int n_at = 0, want = 0;
+            for (int i = 0; i < nt; i++)
+                if (w->fibers[i].state == ST_NAMED_BAR && w->fibers[i].bar_id == id) {
+                    if (want && want != w->fibers[i].bar_n) {
+                        fprintf(stderr, "EMU: %s: threads disagree on the size of named barrier %d\n", t_kernel, id);
+                        abort();
+                    }
+                    want = w->fibers[i].bar_n;
+                    n_at++;
+                }
+            if (want && n_at > want) { fprintf(stderr, "EMU: %s: %d threads at named barrier %d of %d\n", t_kernel, n_at, id, want); abort(); }
+            if (want && n_at == want) {
+                for (int i = 0; i < nt; i++)
+                    if (w->fibers[i].state == ST_NAMED_BAR && w->fibers[i].bar_id == id) w->fibers[i].state = ST_RUN;
                 progress = true;
             }
         }

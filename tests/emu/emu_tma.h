@@ -44,6 +44,7 @@ void tma_store_commit();
 void tma_store_wait_read();
 void tma_store_wait_all();
 static inline void fence_proxy_async() {}
+void named_bar_sync(int id, int n_threads);
 static inline void tma_prefetch_map(const CUtensorMap*) {}
 
 bool fdas_encode_tensor_map(CUtensorMap* out, const void* base, int rank, const uint64_t* dims, const uint64_t* strides_bytes,

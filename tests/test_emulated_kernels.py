@@ -233,7 +233,8 @@ def test_correlate_variants_agree(emu):
     d_S, _ = plan.spectrum(cfg.series())
     planes = {}
     for name, opts in (("packed", {}), ("scalar", {fdas.FDAS_OPT_TUNE_SCALAR: 1}), ("one_chunk", {fdas.FDAS_OPT_TUNE_T_CHUNKS: 1}),
-                       ("five_chunks", {fdas.FDAS_OPT_TUNE_T_CHUNKS: 5})):
+                       ("five_chunks", {fdas.FDAS_OPT_TUNE_T_CHUNKS: 5}), ("staged", {fdas.FDAS_OPT_TUNE_STAGE_TEMPLATES: 1}),
+                       ("staged_one_chunk", {fdas.FDAS_OPT_TUNE_STAGE_TEMPLATES: 1, fdas.FDAS_OPT_TUNE_T_CHUNKS: 1})):
         for k, v in opts.items():
             fdas.fdas_plan_set_option(plan.handle, k, v)
         try:
@@ -242,7 +243,7 @@ def test_correlate_variants_agree(emu):
         finally:
             for k in opts:
                 fdas.fdas_plan_set_option(plan.handle, k, 0)
-    for other in ("scalar", "one_chunk", "five_chunks"):
+    for other in ("scalar", "one_chunk", "five_chunks", "staged", "staged_one_chunk"):
         assert np.array_equal(planes["packed"], planes[other]), other
     thr = oracle.thresholds(16, 1e-3)
     lists = []
@@ -257,6 +258,27 @@ def test_correlate_variants_agree(emu):
                 fdas.fdas_plan_set_option(plan.handle, k, 0)
         lists.append(sorted((int(r["nharm"]), int(r["zi"]), int(r["col"]), float(r["power"])) for r in c))
     assert all(l == lists[0] for l in lists) and len(lists[0]) > 0
+    plan.close()
+
+
+@pytest.mark.parametrize("N,zmax,m,ib,nb", [(1 << 14, 8.0, 64, 1, 1), (1 << 14, 30.0, 256, 0, 2), (1 << 13, 2.0, 1024, 0, 1)])
+def test_staged_templates_kernel(emu, N, zmax, m, ib, nb):
+    """k_correlate_2048_staged (three segments per CTA share every template spectrum through a bulk-copy ring,
+    FDAS_OPT_TUNE_STAGE_TEMPLATES): plane bit for bit the default kernel's, candidates identical; 5 segments (a
+    last CTA with an idle group), interbinning, a batch, one and several template chunks, a ragged last segment."""
+    cfg = synth.small_config(N, zmax, 2.0, m, 2048, interbin=ib, n_dm=nb, n_sig=2, index=51, amp=0.2)
+    xs = np.stack([cfg.series(d) for d in range(nb)])
+    plan = emu.Plan(N, zmax, 2.0, m, 2048, interbin=ib, max_batch=nb, quad_points=512)
+    d_S, _ = plan.spectrum(xs)
+    out = {}
+    for staged in (0, 1):
+        fdas.fdas_plan_set_option(plan.handle, fdas.FDAS_OPT_TUNE_STAGE_TEMPLATES, staged)
+        d_P, d_c, d_n = plan.correlate(d_S, True, 12.0, 1 << 12)
+        out[staged] = (d_P.np().copy(), [cset(d_c.np()[b, :int(d_n.np()[b])]) for b in range(nb)])
+        _, d_c, d_n = plan.correlate(d_S, False, 12.0, 1 << 12)           # fused mode: plane not stored
+        assert [cset(d_c.np()[b, :int(d_n.np()[b])]) for b in range(nb)] == out[staged][1]
+    assert np.array_equal(out[0][0], out[1][0]) and out[0][1] == out[1][1] and sum(len(c) for c in out[0][1]) > 0
+    assert fdas.fdas_plan_status(plan.handle) == 0
     plan.close()
 
 
