@@ -43,19 +43,22 @@ cudaError_t cudaFree(void* p);
 cudaError_t cudaMemcpy(void* d, const void* s, size_t n, cudaMemcpyKind k);
 cudaError_t cudaMemcpyAsync(void* d, const void* s, size_t n, cudaMemcpyKind k, cudaStream_t st);
 cudaError_t cudaMemsetAsync(void* d, int v, size_t n, cudaStream_t st);
-static inline cudaError_t cudaStreamSynchronize(cudaStream_t) { return cudaSuccess; }
+// every stream / event operation is logged (EMU_STREAM_TRACE=<file>) so that a test can rebuild the happens-before graph
+void emu_trace(const char* op, const void* a, const void* b, const void* c, size_t n);
+static inline cudaError_t cudaStreamSynchronize(cudaStream_t s) { emu_trace("streamsync", s, 0, 0, 0); return cudaSuccess; }
 // streams and events: every enqueue runs to completion before it returns, so ordering is trivially kept
 typedef void* cudaEvent_t;
 enum { cudaStreamNonBlocking = 1, cudaEventDisableTiming = 2 };
-static inline cudaError_t cudaStreamCreateWithFlags(cudaStream_t* s, unsigned) { *s = (cudaStream_t)(uintptr_t)0x51; return cudaSuccess; }
+uintptr_t emu_new_id();
+static inline cudaError_t cudaStreamCreateWithFlags(cudaStream_t* s, unsigned) { *s = (cudaStream_t)(0x5000 + emu_new_id()); return cudaSuccess; }
 static inline cudaError_t cudaStreamDestroy(cudaStream_t) { return cudaSuccess; }
-static inline cudaError_t cudaEventCreateWithFlags(cudaEvent_t* e, unsigned) { *e = (cudaEvent_t)(uintptr_t)0xE1; return cudaSuccess; }
+static inline cudaError_t cudaEventCreateWithFlags(cudaEvent_t* e, unsigned) { *e = (cudaEvent_t)(0xE000 + emu_new_id()); return cudaSuccess; }
 static inline cudaError_t cudaEventDestroy(cudaEvent_t) { return cudaSuccess; }
-static inline cudaError_t cudaEventCreate(cudaEvent_t* e) { *e = (cudaEvent_t)(uintptr_t)0xE2; return cudaSuccess; }
+static inline cudaError_t cudaEventCreate(cudaEvent_t* e) { *e = (cudaEvent_t)(0xE000 + emu_new_id()); return cudaSuccess; }
 static inline cudaError_t cudaEventElapsedTime(float* ms, cudaEvent_t, cudaEvent_t) { *ms = 1.0f; return cudaSuccess; }
-static inline cudaError_t cudaEventRecord(cudaEvent_t, cudaStream_t) { return cudaSuccess; }
-static inline cudaError_t cudaEventSynchronize(cudaEvent_t) { return cudaSuccess; }
-static inline cudaError_t cudaStreamWaitEvent(cudaStream_t, cudaEvent_t, unsigned) { return cudaSuccess; }
+static inline cudaError_t cudaEventRecord(cudaEvent_t e, cudaStream_t s) { emu_trace("record", s, e, 0, 0); return cudaSuccess; }
+static inline cudaError_t cudaEventSynchronize(cudaEvent_t e) { emu_trace("eventsync", 0, e, 0, 0); return cudaSuccess; }
+static inline cudaError_t cudaStreamWaitEvent(cudaStream_t s, cudaEvent_t e, unsigned) { emu_trace("wait", s, e, 0, 0); return cudaSuccess; }
 template <class T> static inline cudaError_t cudaMallocHost(T** p, size_t n) { *p = (T*)malloc(n); return *p ? cudaSuccess : cudaErrorMemoryAllocation; }
 static inline cudaError_t cudaFreeHost(void* p) { free(p); return cudaSuccess; }
 static inline cudaError_t cudaGetLastError() { return cudaSuccess; }
@@ -75,7 +78,7 @@ void emu_syncthreads();
 void emu_syncwarp();
 void* emu_dyn_smem();
 void emu_check_ptr(const void* p, size_t n, const char* what);
-void emu_launch(dim3 grid, dim3 block, size_t smem, const char* name, const std::function<void()>& body);
+void emu_launch(dim3 grid, dim3 block, size_t smem, const char* name, const std::function<void()>& body, cudaStream_t st = 0);
 unsigned emu_ballot(int pred);
 static inline unsigned __ballot_sync(unsigned mask, int pred)
 {

@@ -48,8 +48,23 @@ static void guarded_free(void* p)
 cudaError_t cudaMalloc(void** p, size_t n) { *p = guarded_alloc(n); return *p ? cudaSuccess : cudaErrorMemoryAllocation; }
 cudaError_t cudaFree(void* p) { if (p) guarded_free(p); return cudaSuccess; }
 cudaError_t cudaMemcpy(void* d, const void* s, size_t n, cudaMemcpyKind) { memcpy(d, s, n); return cudaSuccess; }
-cudaError_t cudaMemcpyAsync(void* d, const void* s, size_t n, cudaMemcpyKind, cudaStream_t) { memcpy(d, s, n); return cudaSuccess; }
-cudaError_t cudaMemsetAsync(void* d, int v, size_t n, cudaStream_t) { memset(d, v, n); return cudaSuccess; }
+// ---- stream / event trace: "op stream a b n" per line, in host issue order
+static std::atomic<uintptr_t> g_ids{0};
+uintptr_t emu_new_id() { return ++g_ids; }
+void emu_trace(const char* op, const void* a, const void* b, const void* c, size_t n)
+{
+    const char* path = getenv("EMU_STREAM_TRACE");
+    if (!path) return;
+    static std::mutex mu;
+    std::lock_guard<std::mutex> lk(mu);
+    FILE* f = fopen(path, "a");
+    if (!f) return;
+    if (!strcmp(op, "launch")) fprintf(f, "launch %p %s\n", a, (const char*)b);
+    else fprintf(f, "%s %p %p %p %zu\n", op, a, b, c, n);
+    fclose(f);
+}
+cudaError_t cudaMemcpyAsync(void* d, const void* s, size_t n, cudaMemcpyKind, cudaStream_t st) { emu_trace("memcpy", st, d, s, n); memcpy(d, s, n); return cudaSuccess; }
+cudaError_t cudaMemsetAsync(void* d, int v, size_t n, cudaStream_t st) { emu_trace("memset", st, d, 0, n); memset(d, v, n); return cudaSuccess; }
 extern "C" void* emu_malloc(size_t n) { return guarded_alloc(n); }
 extern "C" void emu_free(void* p) { guarded_free(p); }
 
@@ -471,9 +486,10 @@ static void run_block(Worker* w, dim3 block, int order)      // order: 0 forward
 static std::atomic<long> g_launches{0};
 extern "C" long emu_launch_count() { return g_launches.load(); }
 
-void emu_launch(dim3 grid, dim3 block, size_t smem, const char* name, const std::function<void()>& body)
+void emu_launch(dim3 grid, dim3 block, size_t smem, const char* name, const std::function<void()>& body, cudaStream_t st)
 {
     g_launches++;
+    emu_trace("launch", st, name, 0, 0);
     if (getenv("EMU_TRACE"))
         fprintf(stderr, "EMU launch %s grid (%u,%u,%u) block (%u,%u,%u) smem %zu\n", name, grid.x, grid.y, grid.z,
                 block.x, block.y, block.z, smem);

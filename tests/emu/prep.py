@@ -59,7 +59,7 @@ def rewrite(s):
         p1 = match_fwd(s, p0, "(", ")")
         args = s[p0 + 1:p1]
         name = kern.split("<")[0]
-        rep = 'emu_launch(%s, %s, %s, "%s", [&]{ %s(%s); })' % (cfg[0], cfg[1], cfg[2], name, kern, args)
+        rep = 'emu_launch(%s, %s, %s, "%s", [&]{ %s(%s); }, (cudaStream_t)(%s))' % (cfg[0], cfg[1], cfg[2], name, kern, args, cfg[3])
         s = s[:k0] + rep + s[p1 + 1:]
     return s
 

@@ -22,6 +22,7 @@ sys.path.insert(0, os.path.dirname(os.path.abspath(__file__)))
 from emu import harness as E  # noqa: E402
 
 fdas = E.fdas
+ROOT_DIR = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 
 
 @pytest.fixture(params=[("end", "fwd"), ("start", "rev"), ("end", "rand7")],
@@ -428,3 +429,73 @@ sys.exit(10 + L.emu_selftest_tma(int(sys.argv[1])))
     r = run(4)
     assert r.returncode not in (10, 11) and "not aligned" in r.stderr, r.stderr[-300:]
     assert run(5).returncode == 11                                      # buffer reused too early: output corrupted
+
+
+def test_search_host_stream_ordering(tmp_path):
+    """fdas_search_host overlaps the copy of series c+1 with the kernels of series c on three streams; the emulator
+    runs everything synchronously, so the ORDER the library asks for is checked instead: every stream and event
+    call is logged (EMU_STREAM_TRACE), the happens-before graph is rebuilt from stream order, record -> wait pairs
+    and host synchronisations, and every buffer hazard of the pipeline must be ordered by it:
+    the copy into a series buffer after the spectrum kernels that last read it, those kernels after the copy, the
+    counts and candidate copies after the harmonic sum that wrote them, and nothing outstanding at return."""
+    import subprocess
+    trace = str(tmp_path / "trace.txt")
+    prog = r'''
+import os, sys, numpy as np
+sys.path.insert(0, %r); sys.path.insert(0, %r)
+from paper_1511_07343_b200 import synth
+from emu import harness as E
+N = 1 << 13
+x = synth.small_config(N, 8.0, 2.0, 64, 2048, n_sig=2, index=41, amp=0.3).series()
+plan = E.Plan(N, 8.0, 2.0, 64, 2048, quad_points=512)
+open(os.environ["EMU_STREAM_TRACE"], "w").close()                    # drop the plan's own operations
+h_c, h_n = E.fdas.fdas_search_host(plan.handle, np.stack([x] * 6), 4, E.fdas.thresholds(4, 1e-3), 1 << 12)
+assert len(set(h_n.tolist())) == 1 and h_n[0] > 0
+''' % (ROOT_DIR, os.path.dirname(os.path.abspath(__file__)))
+    env = dict(os.environ, EMU_STREAM_TRACE=trace)
+    r = subprocess.run([sys.executable, "-c", prog], capture_output=True, text=True, timeout=600, env=env)
+    assert r.returncode == 0, r.stderr[-800:]
+    ops = [l.split() for l in open(trace) if l.strip()]
+    n = len(ops)
+    anc = [0] * n                                    # bitset of the operations that happen before operation i
+    last_on_stream, last_record, host_before = {}, {}, 0
+    for i, o in enumerate(ops):
+        kind, stream = o[0], o[1]
+        before = host_before                          # whatever the host has synchronised with
+        if kind in ("memcpy", "memset", "launch", "record", "wait"):
+            j = last_on_stream.get(stream)
+            if j is not None:
+                before |= anc[j] | (1 << j)
+            last_on_stream[stream] = i
+        if kind == "wait" and o[2] in last_record:
+            j = last_record[o[2]]
+            before |= anc[j] | (1 << j)
+        if kind == "record":
+            last_record[o[2]] = i
+        anc[i] = before
+        if kind == "eventsync" and o[2] in last_record:
+            j = last_record[o[2]]
+            host_before |= anc[j] | (1 << j)
+        if kind == "streamsync" and stream in last_on_stream:
+            j = last_on_stream[stream]
+            host_before |= anc[j] | (1 << j)
+    hb = lambda a, b: bool(anc[b] >> a & 1)
+    h2d = [i for i, o in enumerate(ops) if o[0] == "memcpy" and int(o[4]) == (1 << 13) * 4]
+    spec_first = [i for i, o in enumerate(ops) if o[0] == "launch" and o[2] == "k_spec_cols"]
+    spec_last = [i for i, o in enumerate(ops) if o[0] == "launch" and o[2] == "k_spec_rows"]
+    harm = [i for i, o in enumerate(ops) if o[0] == "launch" and o[2] == "k_harmsum"]
+    counts = [i for i, o in enumerate(ops) if o[0] == "memcpy" and int(o[4]) == 4]
+    cands = [i for i, o in enumerate(ops) if o[0] == "memcpy" and o[1] not in (ops[spec_first[0]][1], ops[h2d[0]][1])]
+    assert len(h2d) == len(spec_first) == len(spec_last) == len(harm) == len(counts) == len(cands) == 6
+    assert len({ops[i][2] for i in h2d}) == 2                              # two series buffers, alternating
+    for c in range(6):
+        assert ops[h2d[c]][2] == ops[h2d[c % 2]][2]
+        assert hb(h2d[c], spec_first[c]), "spectrum %d may start before its series has arrived" % c
+        if c >= 2:
+            assert hb(spec_last[c - 2], h2d[c]), "series %d may overwrite a buffer the spectrum of %d still reads" % (c, c - 2)
+        if c + 1 < 6:
+            assert not hb(harm[c], h2d[c + 1]), "the copy of series %d is serialised behind the kernels of %d: no overlap" % (c + 1, c)
+        assert hb(harm[c], counts[c]) and hb(counts[c], cands[c]), "candidates of %d copied before they are complete" % c
+    assert all(anc[n - 1] >> i & 1 or i == n - 1 for i in range(n - 1)) or ops[-1][0] == "streamsync"
+    final = host_before
+    assert all(final >> i & 1 for i in h2d + harm + counts + cands), "work outstanding when fdas_search_host returns"
