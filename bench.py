@@ -458,6 +458,7 @@ def run_ours(args):
                         "ms_per_dm": fused_ms, "dm_trials_per_s": world * 1e3 / fused_ms,
                         "frac_of_fft_roofline": t_roof3_ms / fused_ms, "candidates_found": fused_found},
         "candidates_found": n_found,
+        "occupancy": {k: dict(zip(("ctas_per_sm", "registers", "smem_bytes"), fdas.fdas_kernel_occupancy(k))) for k in fdas.OCCUPANCY_KERNELS},
         "gpu_launches": 6 * args.steps,        # 4 spectrum kernels + fused correlate + harmonic sum (+ 1 memset node)
         "plan_status": plan.status(),
         "clocks": clocks,

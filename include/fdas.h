@@ -206,6 +206,13 @@ double fdas_threshold(int32_t n_harm, double pfa);
  * Synchronises `stream`; allocates and frees 4 bytes of device memory.  Not part of the search path. */
 int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, int32_t packed, void* stream);
 
+/* Measurement aid (the occupancy figures DESIGN.md section 6 quotes, from the runtime instead of by hand): resident
+ * CTAs per SM (cudaOccupancyMaxActiveBlocksPerMultiprocessor), registers per thread and static + dynamic shared
+ * memory per CTA of the BASELINE.json configs[2]/[4] instance of a kernel family on the current device.  kernel:
+ * "spec_pass_a", "spec_pass_b", "spec_pass_c", "correlate", "correlate_fused", "correlate_staged", "harmsum"
+ * (FDAS_E_INVALID otherwise).  Not part of the search path. */
+int fdas_kernel_occupancy(const char* kernel, int32_t* ctas_per_sm, int32_t* registers, int32_t* smem_bytes);
+
 int fdas_plan_destroy(fdas_plan* plan);
 
 /* Static text for an FDAS_E_* code; for FDAS_E_CUDA the text of the last CUDA error seen. */

@@ -166,6 +166,19 @@ extern "C" int fdas_plan_status(const fdas_plan* p, uint32_t* out)
     return FDAS_OK;
 }
 
+extern "C" int fdas_kernel_occupancy(const char* kernel, int32_t* ctas_per_sm, int32_t* registers, int32_t* smem_bytes)
+{
+    if (!kernel || !ctas_per_sm || !registers || !smem_bytes) return FDAS_E_INVALID;
+    if (!strcmp(kernel, "spec_pass_a")) return fdas_occupancy_spectrum(0, ctas_per_sm, registers, smem_bytes);
+    if (!strcmp(kernel, "spec_pass_b")) return fdas_occupancy_spectrum(1, ctas_per_sm, registers, smem_bytes);
+    if (!strcmp(kernel, "spec_pass_c")) return fdas_occupancy_spectrum(2, ctas_per_sm, registers, smem_bytes);
+    if (!strcmp(kernel, "correlate")) return fdas_occupancy_correlate(0, ctas_per_sm, registers, smem_bytes);
+    if (!strcmp(kernel, "correlate_fused")) return fdas_occupancy_correlate(1, ctas_per_sm, registers, smem_bytes);
+    if (!strcmp(kernel, "correlate_staged")) return fdas_occupancy_correlate(2, ctas_per_sm, registers, smem_bytes);
+    if (!strcmp(kernel, "harmsum")) return fdas_occupancy_harmsum(ctas_per_sm, registers, smem_bytes);
+    return FDAS_E_INVALID;
+}
+
 extern "C" int fdas_get_templates(const fdas_plan* p, float* h_re_im)
 {
     if (!p || !h_re_im) return FDAS_E_INVALID;

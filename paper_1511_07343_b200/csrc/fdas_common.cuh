@@ -72,6 +72,23 @@ int fdas_launch_resample(fdas_plan* p, const float* d_series, double beta, float
 int fdas_launch_candidates(fdas_plan* p, const float* d_plane, float thr, fdas_cand* d_cands,
                            uint32_t* d_count, uint32_t cap, cudaStream_t st);
 
+// occupancy of the configs[2] instance of a kernel family (fdas_kernel_occupancy): resident CTAs per SM, registers
+// per thread, static + dynamic shared memory per CTA
+template <class K>
+inline int fdas_occupancy_of(K kernel, int threads, size_t dyn_smem, int32_t* ctas, int32_t* regs, int32_t* smem)
+{
+    cudaFuncAttributes fa;
+    int n = 0;
+    if (dyn_smem > 48 * 1024) FDAS_CUDA(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)dyn_smem));
+    FDAS_CUDA(cudaFuncGetAttributes(&fa, kernel));
+    FDAS_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&n, kernel, threads, dyn_smem));
+    *ctas = n; *regs = fa.numRegs; *smem = (int32_t)(fa.sharedSizeBytes + dyn_smem);
+    return FDAS_OK;
+}
+int fdas_occupancy_spectrum(int which, int32_t* ctas, int32_t* regs, int32_t* smem);
+int fdas_occupancy_correlate(int which, int32_t* ctas, int32_t* regs, int32_t* smem);
+int fdas_occupancy_harmsum(int32_t* ctas, int32_t* regs, int32_t* smem);
+
 // ------------------------------------------------------------------ device helpers
 __device__ __forceinline__ float2 cmul(float2 a, float2 b)
 {

@@ -437,3 +437,10 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
     FDAS_LAUNCH_CHECK();
     return FDAS_OK;
 }
+
+int fdas_occupancy_correlate(int which, int32_t* ctas, int32_t* regs, int32_t* smem)
+{
+    if (which == 0) return fdas_occupancy_of(k_correlate_2048<true, false, 1, 7, true>, SEG_THREADS, 0, ctas, regs, smem);
+    if (which == 1) return fdas_occupancy_of(k_correlate_2048<false, true, 1, 7, true>, SEG_THREADS, 0, ctas, regs, smem);
+    return fdas_occupancy_of(k_correlate_2048_staged<true, false, 1, 7, true>, SEG_GROUPS * SEG_THREADS, SEG_STAGED_SMEM, ctas, regs, smem);
+}

@@ -457,3 +457,8 @@ int fdas_launch_candidates(fdas_plan* p, const float* d_plane, float thr, fdas_c
     FDAS_LAUNCH_CHECK();
     return FDAS_OK;
 }
+
+int fdas_occupancy_harmsum(int32_t* ctas, int32_t* regs, int32_t* smem)
+{
+    return fdas_occupancy_of(k_harmsum<5, 4, 3>, 128, 0, ctas, regs, smem);
+}

@@ -402,3 +402,10 @@ int fdas_launch_spectrum_tma(fdas_plan* p, const float* d_series, int n_batch, f
     default: return FDAS_E_INVALID;
     }
 }
+
+int fdas_occupancy_spectrum(int which, int32_t* ctas, int32_t* regs, int32_t* smem)
+{
+    if (which == 0) return fdas_occupancy_of(k_spec_cols<7, true>, SPT_THREADS, 2 * SPT_TILE_BYTES, ctas, regs, smem);
+    if (which == 1) return fdas_occupancy_of(k_spec_cols<7, false>, SPT_THREADS, 2 * SPT_TILE_BYTES, ctas, regs, smem);
+    return fdas_occupancy_of(k_spec_rows<8>, SPT_THREADS, (16 * 258 + 16 * 272) * 8, ctas, regs, smem);
+}

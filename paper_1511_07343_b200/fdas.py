@@ -26,7 +26,7 @@ assert CAND_DTYPE.itemsize == 12
 
 EXPORTS = ["fdas_set_device", "fdas_plan_create", "fdas_plan_set_option", "fdas_plan_info",
            "fdas_build_templates", "fdas_plan_status", "fdas_get_templates", "fdas_spectrum", "fdas_correlate",
-           "fdas_harmsum", "fdas_candidates", "fdas_resample", "fdas_search_host", "fdas_threshold", "fdas_measure_fp32_tflops",
+           "fdas_harmsum", "fdas_candidates", "fdas_resample", "fdas_search_host", "fdas_threshold", "fdas_measure_fp32_tflops", "fdas_kernel_occupancy",
            "fdas_plan_destroy", "fdas_strerror"]
 
 
@@ -69,6 +69,7 @@ def lib():
         L.fdas_resample.argtypes = [vp, vp, f64, vp, vp]
         L.fdas_search_host.argtypes = [vp, vp, i32, i32, vp, vp, vp, u32, vp]
         L.fdas_measure_fp32_tflops.argtypes = [C.POINTER(f64), C.POINTER(f64), i32, vp]
+        L.fdas_kernel_occupancy.argtypes = [C.c_char_p, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
         L.fdas_threshold.argtypes = [i32, f64]
         L.fdas_threshold.restype = f64
         L.fdas_plan_destroy.argtypes = [vp]
@@ -244,6 +245,16 @@ def fdas_measure_fp32_tflops(stream=None, packed=False):
     _check(lib().fdas_measure_fp32_tflops(C.byref(tf), C.byref(ms), 1 if packed else 0, _stream(stream)),
            "fdas_measure_fp32_tflops")
     return tf.value, ms.value
+
+
+OCCUPANCY_KERNELS = ("spec_pass_a", "spec_pass_b", "spec_pass_c", "correlate", "correlate_fused", "correlate_staged", "harmsum")
+
+
+def fdas_kernel_occupancy(kernel: str):
+    """(resident CTAs per SM, registers per thread, shared memory per CTA) of a kernel family's configs[2] instance."""
+    a, b, c = C.c_int32(), C.c_int32(), C.c_int32()
+    _check(lib().fdas_kernel_occupancy(kernel.encode(), C.byref(a), C.byref(b), C.byref(c)), "fdas_kernel_occupancy")
+    return a.value, b.value, c.value
 
 
 def fdas_plan_destroy(plan):

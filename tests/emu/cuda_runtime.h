@@ -70,6 +70,8 @@ int emu_env_int(const char* name, int dflt);
 static inline cudaError_t cudaGetDevice(int* d) { *d = 0; return cudaSuccess; }
 static inline cudaError_t cudaDeviceGetAttribute(int* v, cudaDeviceAttr, int) { *v = emu_env_int("EMU_SMS", 3); return cudaSuccess; }
 template <class F> static inline cudaError_t cudaOccupancyMaxActiveBlocksPerMultiprocessor(int* n, F, int, size_t) { *n = emu_env_int("EMU_CTAS_PER_SM", 2); return cudaSuccess; }
+struct cudaFuncAttributes { int numRegs; size_t sharedSizeBytes; };
+template <class F> static inline cudaError_t cudaFuncGetAttributes(cudaFuncAttributes* a, F) { a->numRegs = 0; a->sharedSizeBytes = 0; return cudaSuccess; }
 static inline const char* cudaGetErrorString(cudaError_t) { return "emu"; }
 template <class F> static inline cudaError_t cudaFuncSetAttribute(F, cudaFuncAttribute, int) { return cudaSuccess; }
 

@@ -27,3 +27,13 @@ def test_fp32_peak_microbenchmark_is_sane(fdas):
     assert 18.0 < tf < 85.0 and ms > 0.0
     tf2, _ = fdas.fdas_measure_fp32_tflops(packed=True)               # FFMA2 chains: same lanes, half the issue slots
     assert 18.0 < tf2 < 170.0
+
+
+def test_occupancy_matches_the_design(fdas):
+    """3 CTAs/SM for the three spectrum passes and the fused segment kernel, 1 for the staged
+    variant (384 threads), 3 CTAs of 4 warps for the harmonic sum -- from the occupancy API, not by hand."""
+    occ = {k: fdas.fdas_kernel_occupancy(k) for k in fdas.OCCUPANCY_KERNELS}
+    print(occ)
+    for k in ("spec_pass_a", "spec_pass_b", "spec_pass_c", "correlate", "correlate_fused", "harmsum"):
+        assert occ[k][0] >= 3, (k, occ[k])
+    assert occ["correlate_staged"][0] == 1 and occ["correlate"][1] <= 168
