@@ -322,6 +322,7 @@ static int launch_cols(const CUtensorMap& in, const CUtensorMap& out, const Spec
 {
     const int smem = 2 * SPT_TILE_BYTES;
     FDAS_CUDA(cudaFuncSetAttribute(k_spec_cols<LR, ACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    FDAS_CUDA(cudaFuncSetAttribute(k_spec_cols<LR, ACC>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));   // 3 CTAs x 72 KB
     k_spec_cols<LR, ACC><<<dim3(a.n_outer * a.n_col_tiles, n_batch), SPT_THREADS, smem, st>>>(in, out, a);
     FDAS_LAUNCH_CHECK();
     return FDAS_OK;
@@ -343,6 +344,7 @@ static int launch_rows(const SpecRowArgs& a, int n_batch, cudaStream_t st)
     constexpr int R = 1 << LR, T = SPT_TILE / R;
     const int smem = (T * (R + 2) + T * (R + R / 16)) * 8;          // a multiple of 128 for every R here
     FDAS_CUDA(cudaFuncSetAttribute(k_spec_rows<LR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    FDAS_CUDA(cudaFuncSetAttribute(k_spec_rows<LR>, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
     k_spec_rows<LR><<<dim3(a.NR / T, n_batch), SPT_THREADS, smem, st>>>(a);
     FDAS_LAUNCH_CHECK();
     return FDAS_OK;
