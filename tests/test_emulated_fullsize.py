@@ -53,3 +53,48 @@ def test_config2_and_config4_at_full_size(monkeypatch):
         assert k in pw and abs(pw[k] - t) <= 1e-4 * t, k
     assert fdas.fdas_plan_status(plan.handle) == 0
     plan.close()
+
+
+def test_config1_interbinned_at_full_size(monkeypatch):
+    """BASELINE.json configs[1]: 2^20 samples, 101 z x 2 template sets (202 templates, 7 chunks), column interleave."""
+    monkeypatch.setenv("EMU_SMS", "148")
+    monkeypatch.setenv("EMU_CTAS_PER_SM", "3")
+    from emu import harness as E
+    cfg = synth.config(1)
+    x = cfg.series()
+    plan = E.Plan(cfg.n_samples, cfg.z_max, cfg.dz, cfg.width, cfg.seg_len, interbin=1)
+    d_S, _ = plan.spectrum(x)
+    d_P, d_c, d_n = plan.correlate(d_S, True, 30.0, 1 << 20)
+    S, _ = oracle.spectrum(x)
+    P_ref = oracle.correlate_fft(S, oracle.templates(cfg.z_max, cfg.dz, cfg.width, 1), cfg.seg_len, interbin=1)
+    P = d_P.np()[0]
+    assert P.shape == (101, 1 << 20)
+    assert not (np.abs(P - P_ref) > 1e-4 * P_ref.max() + 1e-5 * P_ref).any()
+    c_ref = oracle.candidates(P_ref, 30.0)
+    got = {(int(r["zi"]), int(r["col"])) for r in d_c.np()[0, :int(d_n.np()[0])]}
+    assert got == {(int(r["zi"]), int(r["col"])) for r in c_ref} and len(got) > 100
+    plan.close()
+
+
+def test_maximum_series_length(monkeypatch):
+    """2^25 samples (the largest the plan accepts): three passes of 256 x 256 x 256, 2^24 columns per row --
+    index arithmetic at its limits (k h, plane offsets, twiddle exponents), 3 templates."""
+    monkeypatch.setenv("EMU_SMS", "148")
+    monkeypatch.setenv("EMU_CTAS_PER_SM", "3")
+    from emu import harness as E
+    N = 1 << 25
+    x = synth.make_series(N, 77, [synth.Signal(0.02, 9.0e6 + 0.25, 1.5, 0.3), synth.Signal(0.02, 1.6e7 - 3.5, -2.0, 1.0)])
+    plan = E.Plan(N, 2.0, 2.0, 256, 2048)
+    d_S, _ = plan.spectrum(x)
+    d_P, d_c, d_n = plan.correlate(d_S, True, 30.0, 1 << 16)
+    thr = oracle.thresholds(16)
+    c, n = plan.harmsum(d_P, 16, thr, 1 << 20)
+    S, _ = oracle.spectrum(x)
+    P_ref = oracle.correlate_fft(S, oracle.templates(2.0, 2.0, 256), 2048)
+    P = d_P.np()[0]
+    assert not (np.abs(P - P_ref) > 1e-4 * P_ref.max() + 1e-5 * P_ref).any()
+    assert int(d_n.np()[0]) == len(oracle.candidates(P_ref, 30.0)) > 10
+    c_ref = oracle.harmsum(P.astype(np.float64), 16, thr, bin0=1)
+    key = lambda r: (int(r["nharm"]), int(r["zi"]), int(r["col"]))
+    assert {key(q) for q in c} == {key(q) for q in c_ref} and n == len(c_ref) > 100
+    plan.close()
