@@ -261,10 +261,13 @@ __device__ __forceinline__ void correlate_segment(float2* sm, const int tid, con
             for (int j = 0; j < 8; j++) w4[j] = __ldg(Wn + j * SEG_THREADS);
         } else if (stg.producer && t + 2 < t_end) {                               // refill this iteration's slot with template t + 2
             const int b = (t - t_begin) & 1, k = (t - t_begin) >> 1;
-            if (!mbar_wait(stg.empty + b, k & 1, stg.status)) return;
-            mbar_expect_tx(stg.full + b, 8 * SEG_THREADS * 16);
-            tma_load_1d(const_cast<float4*>(stg.wbuf) + b * (8 * SEG_THREADS), Wr + (size_t)(t + 2) * (8 * SEG_THREADS),
-                        8 * SEG_THREADS * 16, stg.full + b);
+            // (on a time-out nothing is issued and nobody leaves alone: every thread then gives up together at the
+            // next wait for this slot, so that no group is left short at its named barrier)
+            if (mbar_wait(stg.empty + b, k & 1, stg.status)) {
+                mbar_expect_tx(stg.full + b, 8 * SEG_THREADS * 16);
+                tma_load_1d(const_cast<float4*>(stg.wbuf) + b * (8 * SEG_THREADS), Wr + (size_t)(t + 2) * (8 * SEG_THREADS),
+                            8 * SEG_THREADS * 16, stg.full + b);
+            }
         }
         group_barrier();
         const int zi = NSET == 1 ? t : (t >> 1), s = NSET == 1 ? 0 : (t & 1);
