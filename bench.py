@@ -329,6 +329,7 @@ def run_ours(args):
     stage = stage_all.mean(axis=0)
     fp32_measured, _ = fdas.fdas_measure_fp32_tflops()       # FFMA-chain microbenchmark (untimed region)
     fp32_packed, _ = fdas.fdas_measure_fp32_tflops(packed=True)
+    l2_gbs = fdas.fdas_measure_l2_gbs()                      # L2 -> SM read bandwidth (untimed region)
     n_found = int(cands[1][0])
     assert plan.status() == 0, "an asynchronous copy timed out in the timed region (fdas_plan_status)"
 
@@ -414,6 +415,7 @@ def run_ours(args):
                                    "achieved_gbs": (plane_bytes + 8 * info.n_bins) / (corr_ms * 1e-3) / 1e9, "peak_gbs": hbm_peak}},
         "harmsum": {"kernels": "k_harmsum<5,4,3>", "bound": "hbm", "ms": hs_ms, "algorithmic_bytes": plane_bytes,
                     "l2_to_sm_bytes_inherent": 5.84 * plane_bytes,    # sum over the 16 streams of (h/16)^2
+                    "l2_measured_gbs": l2_gbs, "frac_of_l2_stream_bound": 5.84 * plane_bytes / (hs_ms * 1e-3) / 1e9 / l2_gbs,
                     "achieved": plane_bytes / (hs_ms * 1e-3) / 1e9, "peak": hbm_peak, "unit": "GB/s"},
     }
     for k in kernels.values():

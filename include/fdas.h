@@ -206,6 +206,12 @@ double fdas_threshold(int32_t n_harm, double pfa);
  * Synchronises `stream`; allocates and frees 4 bytes of device memory.  Not part of the search path. */
 int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, int32_t packed, void* stream);
 
+/* Measurement aid: L2 -> SM read bandwidth in GB/s.  Every CTA (4 per SM) streams the same `bytes`-byte buffer
+ * (1 MB .. 96 MB: L2-resident, far larger than L1) once with coalesced 16-byte loads; best of 3 timed launches with
+ * CUDA events on `stream`.  bench.py reports the harmonic sum's inherent L2 -> SM stream (5.84 x the plane, DESIGN.md
+ * section 6.3) against it.  Synchronises `stream`; allocates and frees `bytes` of device memory.  Not part of the search path. */
+int fdas_measure_l2_gbs(double* out_gbs, size_t bytes, void* stream);
+
 /* Measurement aid (the occupancy figures DESIGN.md section 6 quotes, from the runtime instead of by hand): resident
  * CTAs per SM (cudaOccupancyMaxActiveBlocksPerMultiprocessor), registers per thread and static + dynamic shared
  * memory per CTA of the BASELINE.json configs[2]/[4] instance of a kernel family on the current device.  kernel:

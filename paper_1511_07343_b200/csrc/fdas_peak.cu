@@ -85,3 +85,59 @@ extern "C" int fdas_measure_fp32_tflops(double* out_tflops, double* out_ms, int3
     if (out_ms) *out_ms = best_ms;
     return FDAS_OK;
 }
+
+// L2 -> SM read bandwidth (measurement aid for the harmonic sum, whose inherent cost is an L2 -> SM stream of 5.84
+// planes): EVERY CTA streams the whole buffer -- small enough to stay in the 126 MB L2, far too
+// large for L1 -- once, with coalesced 16-byte loads, each CTA starting at a different place.  Bytes moved from L2
+// = grid x buffer; DRAM is touched on the first pass of the first launch only.
+__global__ void __launch_bounds__(256)
+k_l2_read(const float4* __restrict__ buf, size_t n4, float* __restrict__ sink)
+{
+    float acc = 0.0f;
+    const size_t start = ((size_t)blockIdx.x * 9973u * 256u) % n4;
+    for (size_t i = threadIdx.x; i < n4; i += 256) {
+        size_t j = start + i;
+        if (j >= n4) j -= n4;
+        const float4 v = __ldg(buf + j);
+        acc += v.x + v.y + v.z + v.w;
+    }
+    if (acc == 123.456f) sink[0] = acc;       // never true for a zeroed buffer; keeps the loads alive
+}
+
+extern "C" int fdas_measure_l2_gbs(double* out_gbs, size_t bytes, void* stream)
+{
+    if (!out_gbs || bytes < ((size_t)1 << 20) || bytes > ((size_t)96 << 20)) return FDAS_E_INVALID;
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, sms = 0;
+    FDAS_CUDA(cudaGetDevice(&dev));
+    FDAS_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const size_t n4 = bytes / 16;
+    const int grid = sms * 4;
+    float4* buf = nullptr;
+    float* sink = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaError_t err = cudaMalloc(&buf, n4 * 16);
+    if (err == cudaSuccess) err = cudaMalloc(&sink, sizeof(float));
+    if (err == cudaSuccess) err = cudaMemsetAsync(buf, 0, n4 * 16, st);
+    if (err == cudaSuccess) err = cudaEventCreate(&e0);
+    if (err == cudaSuccess) err = cudaEventCreate(&e1);
+    double best_ms = 1.0e30;
+    for (int rep = 0; rep < 4 && err == cudaSuccess; rep++) {                 // rep 0 warms up
+        err = cudaEventRecord(e0, st);
+        if (err != cudaSuccess) break;
+        k_l2_read<<<grid, 256, 0, st>>>(buf, n4, sink);
+        err = cudaGetLastError();
+        if (err == cudaSuccess) err = cudaEventRecord(e1, st);
+        if (err == cudaSuccess) err = cudaEventSynchronize(e1);
+        float ms = 0.0f;
+        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+        if (err == cudaSuccess && rep > 0 && ms < best_ms) best_ms = ms;
+    }
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
+    if (buf) cudaFree(buf);
+    if (sink) cudaFree(sink);
+    if (err != cudaSuccess) { fdas_set_cuda_error(err, "fdas_measure_l2_gbs"); return FDAS_E_CUDA; }
+    *out_gbs = (double)grid * (double)n4 * 16.0 / (best_ms * 1.0e-3) / 1.0e9;
+    return FDAS_OK;
+}

@@ -26,7 +26,7 @@ assert CAND_DTYPE.itemsize == 12
 
 EXPORTS = ["fdas_set_device", "fdas_plan_create", "fdas_plan_set_option", "fdas_plan_info",
            "fdas_build_templates", "fdas_plan_status", "fdas_get_templates", "fdas_spectrum", "fdas_correlate",
-           "fdas_harmsum", "fdas_candidates", "fdas_resample", "fdas_search_host", "fdas_threshold", "fdas_measure_fp32_tflops", "fdas_kernel_occupancy",
+           "fdas_harmsum", "fdas_candidates", "fdas_resample", "fdas_search_host", "fdas_threshold", "fdas_measure_fp32_tflops", "fdas_measure_l2_gbs", "fdas_kernel_occupancy",
            "fdas_plan_destroy", "fdas_strerror"]
 
 
@@ -69,6 +69,7 @@ def lib():
         L.fdas_resample.argtypes = [vp, vp, f64, vp, vp]
         L.fdas_search_host.argtypes = [vp, vp, i32, i32, vp, vp, vp, u32, vp]
         L.fdas_measure_fp32_tflops.argtypes = [C.POINTER(f64), C.POINTER(f64), i32, vp]
+        L.fdas_measure_l2_gbs.argtypes = [C.POINTER(f64), C.c_size_t, vp]
         L.fdas_kernel_occupancy.argtypes = [C.c_char_p, C.POINTER(i32), C.POINTER(i32), C.POINTER(i32)]
         L.fdas_threshold.argtypes = [i32, f64]
         L.fdas_threshold.restype = f64
@@ -245,6 +246,13 @@ def fdas_measure_fp32_tflops(stream=None, packed=False):
     _check(lib().fdas_measure_fp32_tflops(C.byref(tf), C.byref(ms), 1 if packed else 0, _stream(stream)),
            "fdas_measure_fp32_tflops")
     return tf.value, ms.value
+
+
+def fdas_measure_l2_gbs(nbytes=32 << 20, stream=None):
+    """L2 -> SM read bandwidth (GB/s) of the current device for an L2-resident buffer of `nbytes`."""
+    out = C.c_double()
+    _check(lib().fdas_measure_l2_gbs(C.byref(out), int(nbytes), _stream(stream)), "fdas_measure_l2_gbs")
+    return out.value
 
 
 OCCUPANCY_KERNELS = ("spec_pass_a", "spec_pass_b", "spec_pass_c", "correlate", "correlate_fused", "correlate_staged", "harmsum")

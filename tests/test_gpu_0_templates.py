@@ -25,6 +25,8 @@ def test_fp32_peak_microbenchmark_is_sane(fdas):
     148 SM x 128 lanes x 2 x 1.965 GHz = 74.4 TFLOP/s."""
     tf, ms = fdas.fdas_measure_fp32_tflops()
     assert 18.0 < tf < 85.0 and ms > 0.0
+    l2 = fdas.fdas_measure_l2_gbs()                                      # L2 -> SM: above the HBM copy rate, below 40 TB/s
+    assert 3.0e3 < l2 < 4.0e4
     tf2, _ = fdas.fdas_measure_fp32_tflops(packed=True)               # FFMA2 chains: same lanes, half the issue slots
     assert 18.0 < tf2 < 170.0
 
