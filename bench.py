@@ -331,7 +331,7 @@ def run_ours(args):
     fp32_packed, _ = fdas.fdas_measure_fp32_tflops(packed=True)
     l2_gbs = fdas.fdas_measure_l2_gbs()                      # L2 -> SM read bandwidth (untimed region)
     n_found = int(cands[1][0])
-    assert plan.status() == 0, "an asynchronous copy timed out in the timed region (fdas_plan_status)"
+    assert plan.status() & fdas.FDAS_STATUS_COPY_TIMEOUT == 0, "an asynchronous copy timed out in the timed region (fdas_plan_status)"
 
     # BASELINE.json configs[3] (streaming batch, plane not stored, threshold fused into the segment kernel):
     # a batch of 8 resident DM trials per call, spectrum + fused correlate, reported beside the headline

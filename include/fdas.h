@@ -60,6 +60,9 @@ extern "C" {
 #define FDAS_OPT_TUNE_STAGE_TEMPLATES 107 /* 1: L = 2048 segment kernel with three segments per CTA that share every
                                           * template spectrum through shared memory (one 16 KB bulk copy per CTA and
                                           * template instead of one L2 read per segment); default 0 until it is timed */
+#define FDAS_OPT_TUNE_SPEC_SELFTEST 108 /* before build: 0 = fdas_build_templates checks the TMA-staged spectrum passes against
+                                        * the generic kernels on one seeded series (default), 1 = skip, 2 = test hook:
+                                        * behave as if the check had failed */
 #define FDAS_OPT_TUNE_SPEC_GENERIC 106 /* 1: the generic two-pass spectrum kernels at every length (default: the
                                         * TMA-staged multi-pass transform from 2^13 samples on) */
 
@@ -118,6 +121,8 @@ int fdas_build_templates(fdas_plan* plan, void* stream);
  * a hung GPU; the results of that call are then undefined.  Synchronous (a 4-byte device-to-host copy): call it
  * after synchronising the stream, not in the hot loop. */
 #define FDAS_STATUS_COPY_TIMEOUT 1u
+#define FDAS_STATUS_TMA_FALLBACK 2u   /* the init-stage comparison of the TMA-staged spectrum passes with the generic
+                                       * kernels failed: the plan uses the generic kernels (slower, correct) */
 int fdas_plan_status(const fdas_plan* plan, uint32_t* out);
 
 /* Test hook: copy the fp32 taps to host, h_re_im[(t*m + j)*2 + {0,1}] = {Re, Im} T_t[j].

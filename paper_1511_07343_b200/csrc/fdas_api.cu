@@ -96,6 +96,7 @@ extern "C" int fdas_plan_set_option(fdas_plan* p, int32_t key, int64_t value)
     case FDAS_OPT_TUNE_HS_ROWS:    if (value < 0 || value > 8) return FDAS_E_INVALID; p->tune_hs_rows = (int32_t)value; return FDAS_OK;
     case FDAS_OPT_TUNE_HS_VARIANT: if (value < 0 || value > 1) return FDAS_E_INVALID; p->tune_hs_variant = (int32_t)value; return FDAS_OK;
     case FDAS_OPT_TUNE_STAGE_TEMPLATES: if (value < 0 || value > 1) return FDAS_E_INVALID; p->tune_stage_templates = (int32_t)value; return FDAS_OK;
+    case FDAS_OPT_TUNE_SPEC_SELFTEST: if (value < 0 || value > 2 || p->built) return FDAS_E_INVALID; p->tune_spec_selftest = (int32_t)value; return FDAS_OK;
     case FDAS_OPT_TUNE_SPEC_GENERIC: if (value < 0 || value > 1) return FDAS_E_INVALID; p->tune_spec_generic = (int32_t)value; return FDAS_OK;
     default: break;
     }
@@ -153,6 +154,10 @@ extern "C" int fdas_build_templates(fdas_plan* p, void* stream)
     int rc = fdas_launch_templates(p, st);
     if (rc) return rc;
     FDAS_CUDA(cudaStreamSynchronize(st));
+    if (p->sp_npass && !p->tune_spec_generic && p->tune_spec_selftest != 1) {
+        rc = fdas_spectrum_selftest(p, p->tune_spec_selftest, st);
+        if (rc) return rc;
+    }
     p->built = 1;
     return FDAS_OK;
 }

@@ -13,7 +13,7 @@ struct fdas_plan {
     int32_t built;
     int32_t n_sms;                     // SMs of the device the bank was built on (launch geometry)
     // tuning keys (FDAS_OPT_TUNE_*; 0 = default), read by the launchers
-    int32_t tune_scalar, tune_t_chunks, tune_hs_sectors, tune_hs_rows, tune_hs_variant, tune_spec_generic, tune_stage_templates;
+    int32_t tune_scalar, tune_t_chunks, tune_hs_sectors, tune_hs_rows, tune_hs_variant, tune_spec_generic, tune_stage_templates, tune_spec_selftest;
     // big FFT split of the packed half-length transform: M = n_samples/2 = R1*R2
     int32_t M, R1, R2, C1, C2, n_part;
     size_t  ws_inter_bytes, ws_part_bytes, workspace_bytes;
@@ -53,6 +53,7 @@ int fdas_permute_templates(fdas_plan* p, cudaStream_t st);
 int fdas_launch_spectrum(fdas_plan* p, const float* d_series, int n_batch, float2* d_spec,
                          float* d_meanpow, void* d_ws, cudaStream_t st);
 void fdas_spectrum_tma_plan(fdas_plan* p);
+int fdas_spectrum_selftest(fdas_plan* p, int mode, cudaStream_t st);
 int fdas_launch_spectrum_tma(fdas_plan* p, const float* d_series, int n_batch, float2* d_spec,
                              float* d_meanpow, void* d_ws, cudaStream_t st);
 // series of 2^13 samples and more take the TMA-staged multi-pass transform (tensor maps need 16-byte bases)

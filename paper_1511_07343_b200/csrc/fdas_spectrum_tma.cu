@@ -22,6 +22,7 @@
 #include "fdas_common.cuh"
 #include "fdas_regfft.cuh"
 #include "fdas_tma.cuh"
+#include <string.h>
 
 constexpr int SPT_THREADS = 256;
 constexpr int SPT_TILE = 4096;                       // complex values per tile
@@ -403,6 +404,78 @@ int fdas_launch_spectrum_tma(fdas_plan* p, const float* d_series, int n_batch, f
     case 8: return launch_rows<8>(ra, n_batch, st);
     default: return FDAS_E_INVALID;
     }
+}
+
+// ------------------------------------------------------------------ init-stage self-test
+// The TMA-staged passes have a second, independent implementation of the same transform next to them (the generic
+// kernels).  At plan build -- the "initialization stage", outside every timed region -- both transform
+// one seeded pseudo-random series of the plan's own length and the results are compared on the device.  If the
+// asynchronous-copy path disagrees or one of its waits timed out (a wrong tensor map, a byte count: mistakes that
+// no CPU run can exclude), the plan says so in its status word (FDAS_STATUS_TMA_FALLBACK) and uses the generic
+// kernels from then on: a defect costs speed and is reported, it does not silently corrupt a search.
+__global__ void __launch_bounds__(256)
+k_selftest_fill(float* __restrict__ x, long long n)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        unsigned h = (unsigned)i * 2654435761u;
+        h ^= h >> 15; h *= 2246822519u; h ^= h >> 13;
+        float s, c;
+        sincospif(2.0f * (float)(i & 1023) * (37.0f / 1024.0f), &s, &c);
+        x[i] = (float)(h >> 8) * (1.0f / 8388608.0f) - 1.0f + 0.25f * c;
+    }
+}
+__global__ void __launch_bounds__(256)
+k_selftest_diff(const float* __restrict__ a, const float* __restrict__ b, long long n, unsigned* __restrict__ worst)
+{
+    float m = 0.0f;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const float d = fabsf(a[i] - b[i]);
+        m = (d == d) ? fmaxf(m, d) : 3.0e38f;                          // a NaN counts as the worst possible
+    }
+    atomicMax(worst, __float_as_uint(m));                               // non-negative floats order like their bit patterns
+}
+
+// mode: 0 = run, 2 = pretend the comparison failed (test hook).  Out of memory: the test is skipped.
+int fdas_spectrum_selftest(fdas_plan* p, int mode, cudaStream_t st)
+{
+    if (!p->sp_npass || !p->d_status) return FDAS_OK;
+    const size_t N = (size_t)p->n_samples, M = (size_t)p->M;
+    float* x = nullptr; float2* s1 = nullptr; float2* s2 = nullptr; void* ws = nullptr; unsigned* worst = nullptr;
+    bool mem = cudaMalloc(&x, N * 4) == cudaSuccess && cudaMalloc(&s1, M * 8) == cudaSuccess && cudaMalloc(&s2, M * 8) == cudaSuccess &&
+               cudaMalloc(&ws, p->workspace_bytes) == cudaSuccess && cudaMalloc(&worst, 4) == cudaSuccess;
+    int rc = FDAS_OK;
+    unsigned h_worst = 0, h_status = 0;
+    if (mem) {
+        cudaMemsetAsync(worst, 0, 4, st);
+        k_selftest_fill<<<592, 256, 0, st>>>(x, (long long)N);
+        rc = fdas_launch_spectrum_tma(p, x, 1, s1, nullptr, ws, st);
+        if (rc == FDAS_OK) rc = fdas_launch_spectrum(p, x, 1, s2, nullptr, ws, st);
+        if (rc == FDAS_OK) {
+            k_selftest_diff<<<592, 256, 0, st>>>(reinterpret_cast<const float*>(s1), reinterpret_cast<const float*>(s2), (long long)(2 * M), worst);
+            if (cudaMemcpyAsync(&h_worst, worst, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+                cudaMemcpyAsync(&h_status, p->d_status, 4, cudaMemcpyDeviceToHost, st) != cudaSuccess ||
+                cudaStreamSynchronize(st) != cudaSuccess)
+                rc = FDAS_E_CUDA;
+        }
+    } else {
+        cudaGetLastError();
+    }
+    if (x) cudaFree(x);
+    if (s1) cudaFree(s1);
+    if (s2) cudaFree(s2);
+    if (ws) cudaFree(ws);
+    if (worst) cudaFree(worst);
+    if (rc == FDAS_E_CUDA) { fdas_set_cuda_error(cudaGetLastError(), "fdas_spectrum_selftest"); return rc; }
+    if (!mem || rc != FDAS_OK) return FDAS_OK;                          // could not be run: nothing is concluded
+    float worst_f;
+    memcpy(&worst_f, &h_worst, 4);
+    // both paths are within ~1e-6 of the exact spectrum (|S| ~ 1 after normalisation): 1e-3 is far outside rounding
+    const bool bad = mode == 2 || (h_status & FDAS_STATUS_MBAR_TIMEOUT) || !(worst_f < 1.0e-3f);
+    const uint32_t word = bad ? FDAS_STATUS_TMA_FALLBACK : 0u;
+    if (bad) p->tune_spec_generic = 1;
+    FDAS_CUDA(cudaMemcpyAsync(p->d_status, &word, 4, cudaMemcpyHostToDevice, st));
+    FDAS_CUDA(cudaStreamSynchronize(st));
+    return FDAS_OK;
 }
 
 int fdas_occupancy_spectrum(int which, int32_t* ctas, int32_t* regs, int32_t* smem)

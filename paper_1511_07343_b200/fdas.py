@@ -18,8 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libfdas.so")
 
 FDAS_OK, FDAS_E_INVALID, FDAS_E_STATE, FDAS_E_WORKSPACE, FDAS_E_CUDA, FDAS_E_NOMEM = 0, -1, -2, -3, -4, -5
 FDAS_OPT_INTERBIN, FDAS_OPT_MAX_BATCH, FDAS_OPT_QUAD_POINTS = 1, 2, 3
-FDAS_OPT_TUNE_SCALAR, FDAS_OPT_TUNE_T_CHUNKS, FDAS_OPT_TUNE_HS_SECTORS, FDAS_OPT_TUNE_HS_ROWS, FDAS_OPT_TUNE_HS_VARIANT, FDAS_OPT_TUNE_SPEC_GENERIC, FDAS_OPT_TUNE_STAGE_TEMPLATES = 101, 102, 103, 104, 105, 106, 107
-FDAS_STATUS_COPY_TIMEOUT = 1
+FDAS_OPT_TUNE_SCALAR, FDAS_OPT_TUNE_T_CHUNKS, FDAS_OPT_TUNE_HS_SECTORS, FDAS_OPT_TUNE_HS_ROWS, FDAS_OPT_TUNE_HS_VARIANT, FDAS_OPT_TUNE_SPEC_GENERIC, FDAS_OPT_TUNE_STAGE_TEMPLATES, FDAS_OPT_TUNE_SPEC_SELFTEST = 101, 102, 103, 104, 105, 106, 107, 108
+FDAS_STATUS_COPY_TIMEOUT, FDAS_STATUS_TMA_FALLBACK = 1, 2
 
 CAND_DTYPE = np.dtype([("col", "<i4"), ("zi", "<i2"), ("nharm", "<i2"), ("power", "<f4")])
 assert CAND_DTYPE.itemsize == 12
@@ -278,7 +278,7 @@ class Plan:
     """Owns an fdas_plan handle plus the torch device buffers the hot calls need."""
 
     def __init__(self, n_samples, z_max, dz, template_width, segment_len, interbin=0, max_batch=1,
-                 quad_points=None, device=None):
+                 quad_points=None, device=None, options=()):
         if not torch.cuda.is_available():
             raise RuntimeError("paper_1511_07343_b200 needs a CUDA device (no CPU fallback)")
         self.device = torch.device("cuda", torch.cuda.current_device() if device is None else device)
@@ -290,6 +290,8 @@ class Plan:
             fdas_plan_set_option(self.handle, FDAS_OPT_MAX_BATCH, max_batch)
         if quad_points:
             fdas_plan_set_option(self.handle, FDAS_OPT_QUAD_POINTS, quad_points)
+        for key, value in options:                       # tuning keys that must be set before the build
+            fdas_plan_set_option(self.handle, key, value)
         self.info = fdas_plan_info(self.handle)
         self.max_batch = max_batch
         fdas_build_templates(self.handle)

@@ -65,8 +65,10 @@ def to_dev(a):
 
 
 class Plan:
-    def __init__(self, n_samples, z_max, dz, width, seg_len, interbin=0, max_batch=1, quad_points=None):
+    def __init__(self, n_samples, z_max, dz, width, seg_len, interbin=0, max_batch=1, quad_points=None, options=()):
         self.handle = fdas.fdas_plan_create(n_samples, z_max, dz, width, seg_len)
+        for key, value in options:
+            fdas.fdas_plan_set_option(self.handle, key, value)
         if interbin:
             fdas.fdas_plan_set_option(self.handle, fdas.FDAS_OPT_INTERBIN, 1)
         if max_batch != 1:

@@ -5,7 +5,8 @@ element on the same seeded inputs.  Tolerances are BASELINE.json north_star's:
   candidate (col, zi, nharm) sets identical except entries within 1e-4 relative of the threshold.
 
 Order of the GPU session: the modules are named so that `pytest -m gpu -x` runs every kernel
-family at config-0 size first (test_gpu_0_* ... test_gpu_4_*) and the full-size cases (2^20 ... 2^25 samples) last
+family at config-0 size first (test_gpu_0_* ... test_gpu_4_*), then the strict checks of the asynchronous-copy
+paths (test_gpu_5_async_copies.py), and the full-size cases (2^20 ... 2^25 samples) last
 (test_gpu_9_fullsize.py); the first failure stops the run.
 """
 import numpy as np

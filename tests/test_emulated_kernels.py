@@ -101,6 +101,29 @@ def test_spectrum_paths_agree_and_fall_back(emu):
     plan.close()
 
 
+def test_spectrum_selftest_and_fallback(emu):
+    """fdas_build_templates compares the TMA-staged passes with the generic kernels on one seeded series: in the
+    normal case the status word stays 0 and the TMA passes are used; if the comparison fails (test hook: option
+    value 2) the plan reports FDAS_STATUS_TMA_FALLBACK and its spectra are the generic kernels', bit for bit."""
+    N = 1 << 14
+    x = synth.make_series(N, 321)
+    ok = emu.Plan(N, 4.0, 2.0, 16, 256, quad_points=64)
+    assert fdas.fdas_plan_status(ok.handle) == 0
+    spec = lambda plan: (lambda d: d[0].np().copy())(plan.spectrum(x))     # (the buffers stay alive while they are copied)
+    S_tma = spec(ok)
+    fdas.fdas_plan_set_option(ok.handle, fdas.FDAS_OPT_TUNE_SPEC_GENERIC, 1)
+    S_gen = spec(ok)
+    ok.close()
+    bad = emu.Plan(N, 4.0, 2.0, 16, 256, quad_points=64, options=[(fdas.FDAS_OPT_TUNE_SPEC_SELFTEST, 2)])
+    assert fdas.fdas_plan_status(bad.handle) == fdas.FDAS_STATUS_TMA_FALLBACK
+    S_bad = spec(bad)
+    bad.close()
+    assert np.array_equal(S_bad, S_gen) and not np.array_equal(S_tma, S_gen)
+    skipped = emu.Plan(N, 4.0, 2.0, 16, 256, quad_points=64, options=[(fdas.FDAS_OPT_TUNE_SPEC_SELFTEST, 1)])
+    assert fdas.fdas_plan_status(skipped.handle) == 0 and np.array_equal(spec(skipped), S_tma)
+    skipped.close()
+
+
 def test_all_zero_series(emu):
     """Degenerate input (G22): zero spectrum, zero plane, no candidates, nothing NaN."""
     N = 1 << 13
