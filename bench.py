@@ -235,9 +235,13 @@ def run_ab(args):
         return e0.elapsed_time(e1) / args.steps
 
     corr = lambda: fdas.fdas_correlate(plan.handle, d_spec, 1, d_plane, 0.0, None, None, 0)
+    spec = lambda: fdas.fdas_spectrum(plan.handle, d_x, 1, d_spec, d_mu, plan.workspace)
     hs = lambda: fdas.fdas_harmsum(plan.handle, d_plane[0], 16, thr, cands[0], cands[1], cap)
-    out = {"correlate_ms": {}, "harmsum_ms": {}, "steps": args.steps}
+    out = {"spectrum_ms": {}, "correlate_ms": {}, "harmsum_ms": {}, "steps": args.steps, "plan_status": plan.status()}
     F = fdas
+    for name, opts in (("tma_3pass", {}), ("generic_2pass", {F.FDAS_OPT_TUNE_SPEC_GENERIC: 1})):
+        out["spectrum_ms"][name] = timed(spec, opts)
+    spec()
     for name, opts in (("packed", {}), ("scalar", {F.FDAS_OPT_TUNE_SCALAR: 1}),
                        ("packed_1chunk", {F.FDAS_OPT_TUNE_T_CHUNKS: 1}), ("packed_2chunks", {F.FDAS_OPT_TUNE_T_CHUNKS: 2}),
                        ("packed_4chunks", {F.FDAS_OPT_TUNE_T_CHUNKS: 4}), ("packed_6chunks", {F.FDAS_OPT_TUNE_T_CHUNKS: 6}),

@@ -14,7 +14,7 @@ cd "${GRAFT_REPO_ROOT:-$(dirname "$0")/..}" || exit 9
 O=gpurun_out
 mkdir -p $O
 stage=${1:-tests}
-SMALL="tests/test_gpu_0_templates.py tests/test_gpu_1_spectrum.py tests/test_gpu_2_correlate.py tests/test_gpu_3_harmsum.py tests/test_gpu_4_host_resample.py"
+SMALL="tests/test_gpu_0_templates.py tests/test_gpu_1_spectrum.py tests/test_gpu_2_correlate.py tests/test_gpu_3_harmsum.py tests/test_gpu_4_host_resample.py tests/test_gpu_5_async_copies.py"
 {
 nvidia-smi --query-gpu=name,driver_version,clocks.max.sm,memory.total --format=csv
 git rev-parse --short HEAD 2>/dev/null
