@@ -214,7 +214,8 @@ k_spec_rows(SpecRowArgs a)
     float2* tin = dsm;                               // [T][PITCH]: the rows, later their transforms
     float2* ex = dsm + T * PITCH;                    // [T][XP]
     __shared__ __align__(8) uint64_t bar;
-    __shared__ float2 twr[R];
+    __shared__ float2 twr[R];                        // W_R^x
+    __shared__ float2 twu[R];                        // W_{2R}^x = W_N^{NR x}: the k_c part of the untangle twiddle
     const int tid = threadIdx.x, rho = tid / P, t = tid % P;
     const int bt = blockIdx.y, item = blockIdx.x;
     const int NR = a.NR, M = a.M;
@@ -232,7 +233,10 @@ k_spec_rows(SpecRowArgs a)
         const float2* base = a.src + (size_t)bt * M;
         for (int s = 0; s < T; s++) tma_load_1d(tin + s * PITCH, base + (size_t)row_of(s) * R, R * 8, &bar);
     }
-    if (tid < R) twr[tid] = twiddle(tid, R, -1.0f);
+    if (tid < R) {
+        twr[tid] = twiddle(tid, R, -1.0f);
+        twu[tid] = twiddle(tid, 2 * R, -1.0f);
+    }
     if (!mbar_wait(&bar, 0, a.status)) return;
 
     float2 v[16];
@@ -262,14 +266,16 @@ k_spec_rows(SpecRowArgs a)
     const int pr = tid % H, ka = item * H + pr;
     const float2* ra = tin + pr * PITCH;             // row kappa
     const float2* rb = tin + (H + pr) * PITCH;       // its partner (or, for kappa = 0, row NR/2)
+    // W_N^k, k = kappa + NR kc, as W_N^kappa (one sincospif per thread) times W_{2 Rc}^kc (table): N = 2 NR Rc
     const int N = 2 * M;
+    const float2 wka = twiddle(ka, N, -1.0f), whalf = twiddle(1, 4 * R, -1.0f);     // W_N^{NR/2} = W_{4 Rc}
     for (int kc = tid / H; kc < R; kc += SPT_THREADS / H) {
         if (ka != 0) {
             const float2 za = ra[kc], zb = rb[R - 1 - kc];           // Z_k, Z_{M-k},  k = kappa + NR kc
             const int k = ka + NR * kc;
             const float2 e = make_float2(0.5f * (za.x + zb.x), 0.5f * (za.y - zb.y));       // (Z_k + conj Z_{M-k})/2
             const float2 d = make_float2(0.5f * (za.x - zb.x), 0.5f * (za.y + zb.y));       // (Z_k - conj Z_{M-k})/2
-            const float2 p = cmul(make_float2(d.y, -d.x), twiddle(k, N, -1.0f));            // W_N^k O_k,  O = -i d
+            const float2 p = cmul(make_float2(d.y, -d.x), cmul(wka, twu[kc]));               // W_N^k O_k,  O = -i d
             out[k - 1] = make_float2((e.x + p.x) * sc, (e.y + p.y) * sc);                  // F_k
             out[M - k - 1] = make_float2((e.x - p.x) * sc, -(e.y - p.y) * sc);             // F_{M-k} = conj(E - W O)
         } else {
@@ -281,14 +287,14 @@ k_spec_rows(SpecRowArgs a)
                 const int k = NR * kc;
                 const float2 e = make_float2(0.5f * (z0.x + z0p.x), 0.5f * (z0.y - z0p.y));
                 const float2 d = make_float2(0.5f * (z0.x - z0p.x), 0.5f * (z0.y + z0p.y));
-                const float2 p = cmul(make_float2(d.y, -d.x), twiddle(k, N, -1.0f));
+                const float2 p = cmul(make_float2(d.y, -d.x), twu[kc]);                       // k = NR kc
                 out[k - 1] = make_float2((e.x + p.x) * sc, (e.y + p.y) * sc);
             }
             const float2 zh = rb[kc], zhp = rb[R - 1 - kc];
             const int k = NR / 2 + NR * kc;
             const float2 e = make_float2(0.5f * (zh.x + zhp.x), 0.5f * (zh.y - zhp.y));
             const float2 d = make_float2(0.5f * (zh.x - zhp.x), 0.5f * (zh.y + zhp.y));
-            const float2 p = cmul(make_float2(d.y, -d.x), twiddle(k, N, -1.0f));
+            const float2 p = cmul(make_float2(d.y, -d.x), cmul(whalf, twu[kc]));              // k = NR/2 + NR kc
             out[k - 1] = make_float2((e.x + p.x) * sc, (e.y + p.y) * sc);
         }
     }
