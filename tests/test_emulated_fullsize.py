@@ -7,6 +7,7 @@ import os
 import sys
 
 import numpy as np
+import pytest
 
 import oracle
 from paper_1511_07343_b200 import synth
@@ -55,6 +56,7 @@ def test_config2_and_config4_at_full_size(monkeypatch):
     plan.close()
 
 
+@pytest.mark.skipif(not os.environ.get("FDAS_EMU_ALL"), reason="a minute of oracle time: run with FDAS_EMU_ALL=1 (profiles/r2_emulator_fullsize.md)")
 def test_config1_interbinned_at_full_size(monkeypatch):
     """BASELINE.json configs[1]: 2^20 samples, 101 z x 2 template sets (202 templates, 7 chunks), column interleave."""
     monkeypatch.setenv("EMU_SMS", "148")
