@@ -139,6 +139,7 @@ extern "C" int fdas_build_templates(fdas_plan* p, void* stream)
     if (!p->d_taps && cudaMalloc(&p->d_taps, (size_t)p->n_t * p->m * sizeof(float2)) != cudaSuccess) { p->d_taps = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
     if (!p->d_W && cudaMalloc(&p->d_W, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { p->d_W = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
     if (!p->d_Wr && cudaMalloc(&p->d_Wr, (size_t)p->n_t * p->L * sizeof(float2)) != cudaSuccess) { p->d_Wr = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
+    if (!p->d_segtw && cudaMalloc(&p->d_segtw, 46 * 128 * sizeof(float2)) != cudaSuccess) { p->d_segtw = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
     if (!p->d_status) {
         if (cudaMalloc(&p->d_status, sizeof(uint32_t)) != cudaSuccess) { p->d_status = nullptr; cudaGetLastError(); return FDAS_E_NOMEM; }
         FDAS_CUDA(cudaMemsetAsync(p->d_status, 0, sizeof(uint32_t), st));

@@ -24,6 +24,7 @@ struct fdas_plan {
     float2* d_taps;   // [n_t][m]  conj R_z(d_j), fp32
     float2* d_W;      // [n_t][L]  FFT_L(index-reversed taps)/L, natural order
     float2* d_Wr;     // the same spectra in the register layout of k_correlate_2048 (L = 2048 only)
+    float2* d_segtw;  // per-thread twiddle table of the L = 2048 segment kernels (46 x 128 float2, fdas_correlate.cu)
     // scratch arena of fdas_search_host (device, owned, lazily allocated)
     void*   arena;
     size_t  arena_bytes;

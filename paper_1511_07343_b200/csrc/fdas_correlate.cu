@@ -129,6 +129,44 @@ __device__ __forceinline__ void seg_pass3(const float2* buf, const float2* tw_a,
     }
 }
 
+// Per-thread constants of the segment kernels: the 14 + 15 twiddles of the forward transform and the 16 of the inverse
+// passes depend on the thread index only, so they are computed ONCE with the bank (same device functions: the planes do
+// not change by a bit) instead of 45 sincospif per thread in the prologue of every CTA (~1350 of its ~2000 instructions,
+// i.e. ~8 % of a 29-template CTA).  Entry e of thread tid is the float2 half (e & 1) of table[(e >> 1) * 128 + tid]:
+//   e =  0..6   exp(-2 pi i k3 tid / 2048),         k3 = 1..7        (forward pass over n3, p = tid)
+//   e =  7..13  exp(-2 pi i k3 (tid + 128) / 2048)                    (p = tid + 128)
+//   e = 14..28  exp(-2 pi i k2 lo / 256),           k2 = 1..15, lo = tid & 15
+//   e = 29..36  make_tw<16>(lo, 256);  e = 37..40  make_tw<8>(2 tid, 2048);  e = 41..44  make_tw<8>(2 tid + 1, 2048)
+constexpr int SEG_TW_ENTRIES = 46;                 // 45 used, padded to whole float4
+constexpr int SEG_TW_FLOAT4 = SEG_TW_ENTRIES / 2 * SEG_THREADS;
+
+__global__ void __launch_bounds__(SEG_THREADS)
+k_segment_twiddles(float4* __restrict__ table)
+{
+    const int tid = threadIdx.x, lo = tid & 15;
+    float2 e[SEG_TW_ENTRIES];
+#pragma unroll
+    for (int k3 = 1; k3 < 8; k3++) {
+        e[k3 - 1] = twiddle(k3 * tid, 2048, -1.0f);
+        e[6 + k3] = twiddle(k3 * (tid + 128), 2048, -1.0f);
+    }
+#pragma unroll
+    for (int k2 = 1; k2 < 16; k2++) e[13 + k2] = twiddle(k2 * lo, 256, -1.0f);
+    make_tw<16>(e + 29, lo, 256);
+    make_tw<8>(e + 37, 2 * tid, 2048);
+    make_tw<8>(e + 41, 2 * tid + 1, 2048);
+    e[45] = make_float2(0.0f, 0.0f);
+#pragma unroll
+    for (int j = 0; j < SEG_TW_ENTRIES / 2; j++) table[j * SEG_THREADS + tid] = make_float4(e[2 * j].x, e[2 * j].y, e[2 * j + 1].x, e[2 * j + 1].y);
+}
+
+// entry e (compile time after unrolling) of this thread; the two halves of a float4 share one load
+__device__ __forceinline__ float2 seg_tw(const float4* __restrict__ table, int tid, int e)
+{
+    const float4 q = __ldg(table + (e >> 1) * SEG_THREADS + tid);
+    return (e & 1) ? make_float2(q.z, q.w) : make_float2(q.x, q.y);
+}
+
 // Shared state of the STAGED variant (k_correlate_2048_staged): NG segments ("groups" of 128 threads) per CTA take
 // every template spectrum from a two-slot ring in shared memory that ONE thread fills with 16 KB bulk copies
 // (cp.async.bulk, fdas_tma.cuh).  full[b]: the copy into slot b has landed (1 arrival + 16384 bytes);
@@ -148,9 +186,10 @@ struct SegStage {
 template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK, int NG>
 __device__ __forceinline__ void correlate_segment(float2* sm, const int tid, const int seg, const int bt, const int t_begin,
                                                   const int t_end, const float2* __restrict__ spec,
-                                                  const float4* __restrict__ Wr, float* __restrict__ plane,
-                                                  fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap,
-                                                  float thr, int n_bins, int n_z, int m, int step, const SegStage& stg)
+                                                  const float4* __restrict__ Wr, const float4* __restrict__ twt,
+                                                  float* __restrict__ plane, fdas_cand* __restrict__ cands,
+                                                  uint32_t* __restrict__ counts, uint32_t cap, float thr, int n_bins, int n_z,
+                                                  int m, int step, const SegStage& stg)
 {
     constexpr int L = 2048;
     constexpr int nset = NSET;
@@ -177,7 +216,7 @@ __device__ __forceinline__ void correlate_segment(float2* sm, const int tid, con
             dit_const<8, -1, PK>(u);
 #pragma unroll
             for (int k3 = 0; k3 < 8; k3++) {
-                float2 val = k3 ? cmul(u[k3], twiddle(k3 * p, L, -1.0f)) : u[0];
+                float2 val = k3 ? cmul(u[k3], seg_tw(twt, tid, 7 * g + k3 - 1)) : u[0];
                 buf[p + SEG_PITCH3 * k3] = val;
             }
         }
@@ -187,7 +226,7 @@ __device__ __forceinline__ void correlate_segment(float2* sm, const int tid, con
         for (int n2 = 0; n2 < 16; n2++) v[bitrev(n2, 4)] = buf[lo + 16 * n2 + SEG_PITCH3 * k3A];
         dit_const<16, -1, PK>(v);
 #pragma unroll
-        for (int k2 = 1; k2 < 16; k2++) v[k2] = cmul(v[k2], twiddle(k2 * lo, 256, -1.0f));
+        for (int k2 = 1; k2 < 16; k2++) v[k2] = cmul(v[k2], seg_tw(twt, tid, 13 + k2));
         __syncwarp();
 #pragma unroll
         for (int k2 = 0; k2 < 16; k2++) buf[k2 + 18 * lo + SEG_PITCH3 * k3A] = v[k2];
@@ -200,10 +239,14 @@ __device__ __forceinline__ void correlate_segment(float2* sm, const int tid, con
         group_barrier();
     }
 
-    float2 tw2[8], tw3[2][4];
-    make_tw<16>(tw2, lo, 256);
-    make_tw<8>(tw3[0], 2 * tid, L);
-    make_tw<8>(tw3[1], 2 * tid + 1, L);
+    float2 tw2[8], tw3[2][4];                                      // inverse-pass twiddles (loop invariant), from the table
+#pragma unroll
+    for (int i = 0; i < 8; i++) tw2[i] = seg_tw(twt, tid, 29 + i);
+#pragma unroll
+    for (int i = 0; i < 4; i++) {
+        tw3[0][i] = seg_tw(twt, tid, 37 + i);
+        tw3[1][i] = seg_tw(twt, tid, 41 + i);
+    }
 
     const size_t n_cols = (size_t)n_bins * nset;
     const int omax = min(step, n_bins - c0);                       // even: step, n_bins and c0 are even
@@ -284,15 +327,15 @@ __device__ __forceinline__ void correlate_segment(float2* sm, const int tid, con
 
 template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK>
 __global__ void __launch_bounds__(SEG_THREADS, 3)
-k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
-                    fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
-                    int n_bins, int n_z, int m, int step, int t_chunk)
+k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr, const float4* __restrict__ twt,
+                 float* __restrict__ plane, fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
+                 int n_bins, int n_z, int m, int step, int t_chunk)
 {
     __shared__ __align__(16) float2 sm[2 * SEG_BUF];
     const int n_t = n_z * NSET;
     const int t_begin = blockIdx.y * t_chunk, t_end = min(n_t, t_begin + t_chunk);
     correlate_segment<HAS_PLANE, HAS_CANDS, NSET, NKEEP, PK, 1>(sm, threadIdx.x, blockIdx.x, blockIdx.z, t_begin, t_end, spec, Wr,
-                                                                 plane, cands, counts, cap, thr, n_bins, n_z, m, step, SegStage{});
+                                                                 twt, plane, cands, counts, cap, thr, n_bins, n_z, m, step, SegStage{});
 }
 
 // STAGED variant (tuning key FDAS_OPT_TUNE_STAGE_TEMPLATES; SURVEY section 7 hard part 2, "several segments per
@@ -308,8 +351,8 @@ constexpr int SEG_STAGED_SMEM = SEG_RING_BYTES + SEG_GROUPS * 2 * SEG_BUF * 8 + 
 
 template <bool HAS_PLANE, bool HAS_CANDS, int NSET, int NKEEP, bool PK>
 __global__ void __launch_bounds__(SEG_GROUPS* SEG_THREADS, 1)
-k_correlate_2048_staged(const float2* __restrict__ spec, const float4* __restrict__ Wr, float* __restrict__ plane,
-                        fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
+k_correlate_2048_staged(const float2* __restrict__ spec, const float4* __restrict__ Wr, const float4* __restrict__ twt,
+                        float* __restrict__ plane, fdas_cand* __restrict__ cands, uint32_t* __restrict__ counts, uint32_t cap, float thr,
                         int n_bins, int n_z, int m, int step, int t_chunk, int n_seg, uint32_t* status)
 {
     extern __shared__ __align__(128) float2 dsm[];
@@ -340,8 +383,8 @@ k_correlate_2048_staged(const float2* __restrict__ spec, const float4* __restric
     const int seg = blockIdx.x * SEG_GROUPS + group;
     if (seg < n_seg) {
         correlate_segment<HAS_PLANE, HAS_CANDS, NSET, NKEEP, PK, SEG_GROUPS>(exch + group * 2 * SEG_BUF, tid, seg, blockIdx.z, t_begin,
-                                                                           t_end, spec, Wr, plane, cands, counts, cap, thr, n_bins,
-                                                                           n_z, m, step, stg);
+                                                                           t_end, spec, Wr, twt, plane, cands, counts, cap, thr,
+                                                                           n_bins, n_z, m, step, stg);
     } else {                                   // no segment: consume the ring so that the producer's waits complete
         for (int t = t_begin; t < t_end; t++) {
             const int b = (t - t_begin) & 1, k = (t - t_begin) >> 1;
@@ -370,6 +413,8 @@ int fdas_permute_templates(fdas_plan* p, cudaStream_t st)
     int n = p->n_t * 8 * SEG_THREADS;
     k_permute_templates_2048<<<(n + 255) / 256, 256, 0, st>>>(p->d_W, reinterpret_cast<float4*>(p->d_Wr), p->n_t);
     FDAS_LAUNCH_CHECK();
+    k_segment_twiddles<<<1, SEG_THREADS, 0, st>>>(reinterpret_cast<float4*>(p->d_segtw));
+    FDAS_LAUNCH_CHECK();
     return FDAS_OK;
 }
 
@@ -388,7 +433,7 @@ int fdas_launch_correlate(fdas_plan* p, const float2* d_spec, int n_batch, float
         int t_chunk = (p->n_t + n_chunk - 1) / n_chunk;
         n_chunk = (p->n_t + t_chunk - 1) / t_chunk;
         dim3 grid(p->n_seg, n_chunk, n_batch);
-#define FDAS_SEG_ARGS d_spec, reinterpret_cast<const float4*>(p->d_Wr), d_plane, d_cands, d_counts, cap, thr, \
+#define FDAS_SEG_ARGS d_spec, reinterpret_cast<const float4*>(p->d_Wr), reinterpret_cast<const float4*>(p->d_segtw), d_plane, d_cands, d_counts, cap, thr, \
                       (int)p->n_bins, p->n_z, p->m, p->step, t_chunk
 #define FDAS_SEG_LAUNCH(...)                                                                                        \
         if (d_plane && d_cands) k_correlate_2048<true, true, __VA_ARGS__><<<grid, SEG_THREADS, 0, st>>>(FDAS_SEG_ARGS); \

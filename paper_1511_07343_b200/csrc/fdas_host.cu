@@ -162,6 +162,7 @@ extern "C" int fdas_plan_destroy(fdas_plan* p)
     if (p->d_W) cudaFree(p->d_W);
     if (p->d_Wr) cudaFree(p->d_Wr);
     if (p->d_status) cudaFree(p->d_status);
+    if (p->d_segtw) cudaFree(p->d_segtw);
     if (p->arena) cudaFree(p->arena);
     if (p->pinned_counts) cudaFreeHost(p->pinned_counts);
     if (p->pipe_ready) {
