@@ -245,8 +245,8 @@ def run_ab(args):
     for name, opts in (("packed", {}), ("scalar", {F.FDAS_OPT_TUNE_SCALAR: 1}),
                        ("packed_1chunk", {F.FDAS_OPT_TUNE_T_CHUNKS: 1}), ("packed_2chunks", {F.FDAS_OPT_TUNE_T_CHUNKS: 2}),
                        ("packed_4chunks", {F.FDAS_OPT_TUNE_T_CHUNKS: 4}), ("packed_6chunks", {F.FDAS_OPT_TUNE_T_CHUNKS: 6}),
-                       ("staged_3seg", {F.FDAS_OPT_TUNE_STAGE_TEMPLATES: 1}),
-                       ("staged_3seg_1chunk", {F.FDAS_OPT_TUNE_STAGE_TEMPLATES: 1, F.FDAS_OPT_TUNE_T_CHUNKS: 1})):
+                       ("staged_4seg", {F.FDAS_OPT_TUNE_STAGE_TEMPLATES: 1}),
+                       ("staged_4seg_1chunk", {F.FDAS_OPT_TUNE_STAGE_TEMPLATES: 1, F.FDAS_OPT_TUNE_T_CHUNKS: 1})):
         out["correlate_ms"][name] = timed(corr, opts)
     corr()
     for name, opts in (("S16", {}), ("S1", {F.FDAS_OPT_TUNE_HS_SECTORS: 1}), ("S8", {F.FDAS_OPT_TUNE_HS_SECTORS: 8}),

@@ -57,7 +57,7 @@ extern "C" {
 #define FDAS_OPT_TUNE_HS_SECTORS 103  /* angular sectors of the harmonic-sum tile order, 1..64 (default 16) */
 #define FDAS_OPT_TUNE_HS_ROWS    104  /* warps per CTA of the harmonic-sum kernel, 1..8 (default 4) */
 #define FDAS_OPT_TUNE_HS_VARIANT 105  /* 1: 128-column harmonic-sum tiles (default 64) */
-#define FDAS_OPT_TUNE_STAGE_TEMPLATES 107 /* 1: L = 2048 segment kernel with three segments per CTA that share every
+#define FDAS_OPT_TUNE_STAGE_TEMPLATES 107 /* 1: L = 2048 segment kernel with four segments per CTA that share every
                                           * template spectrum through shared memory (one 16 KB bulk copy per CTA and
                                           * template instead of one L2 read per segment); default 0 until it is timed */
 #define FDAS_OPT_TUNE_SPEC_SELFTEST 108 /* before build: 0 = fdas_build_templates checks the TMA-staged spectrum passes against

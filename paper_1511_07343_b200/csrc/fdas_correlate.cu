@@ -341,11 +341,11 @@ k_correlate_2048(const float2* __restrict__ spec, const float4* __restrict__ Wr,
 // STAGED variant (tuning key FDAS_OPT_TUNE_STAGE_TEMPLATES; SURVEY section 7 hard part 2, "several segments per
 // template load"): one CTA = SEG_GROUPS groups of 128 threads = SEG_GROUPS adjacent segments; every template
 // spectrum crosses L2 -> SM ONCE per CTA, as a 16 KB bulk copy (UBLKCP) into a two-slot ring, instead of once
-// per segment: 1.1 GB instead of up to 3.3 GB per DM trial at configs[2], whatever L1 does.  Groups run
+// per segment: 0.8 GB instead of up to 3.3 GB per DM trial at configs[2], whatever L1 does.  Groups run
 // independently between ring accesses (their own exchange buffers and named barrier).  A group whose segment
 // lies beyond the series (last CTA) only keeps the ring protocol going.
 // dynamic shared memory: ring [2][16 KB] | exchange buffers [SEG_GROUPS][2][SEG_BUF] | 4 mbarriers.
-constexpr int SEG_GROUPS = 3;
+constexpr int SEG_GROUPS = 4;
 constexpr int SEG_RING_BYTES = 2 * 8 * SEG_THREADS * 16;
 constexpr int SEG_STAGED_SMEM = SEG_RING_BYTES + SEG_GROUPS * 2 * SEG_BUF * 8 + 128;
 

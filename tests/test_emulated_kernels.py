@@ -287,9 +287,9 @@ def test_correlate_variants_agree(emu):
 
 @pytest.mark.parametrize("N,zmax,m,ib,nb", [(1 << 14, 8.0, 64, 1, 1), (1 << 14, 30.0, 256, 0, 2), (1 << 13, 2.0, 1024, 0, 1)])
 def test_staged_templates_kernel(emu, N, zmax, m, ib, nb):
-    """k_correlate_2048_staged (three segments per CTA share every template spectrum through a bulk-copy ring,
+    """k_correlate_2048_staged (four segments per CTA share every template spectrum through a bulk-copy ring,
     FDAS_OPT_TUNE_STAGE_TEMPLATES): plane bit for bit the default kernel's, candidates identical; 5 segments (a
-    last CTA with an idle group), interbinning, a batch, one and several template chunks, a ragged last segment."""
+    last CTA with idle groups), interbinning, a batch, one and several template chunks, a ragged last segment."""
     cfg = synth.small_config(N, zmax, 2.0, m, 2048, interbin=ib, n_dm=nb, n_sig=2, index=51, amp=0.2)
     xs = np.stack([cfg.series(d) for d in range(nb)])
     plan = emu.Plan(N, zmax, 2.0, m, 2048, interbin=ib, max_batch=nb, quad_points=512)

@@ -28,7 +28,7 @@ def test_tma_spectrum_is_in_use_and_right(fdas, log2n):
 
 
 def test_staged_segment_kernel(fdas):
-    """FDAS_OPT_TUNE_STAGE_TEMPLATES: three segments per CTA share each template spectrum through a bulk-copy ring;
+    """FDAS_OPT_TUNE_STAGE_TEMPLATES: four segments per CTA share each template spectrum through a bulk-copy ring;
     plane and candidates bit for bit the default kernel's (5 segments: an idle group; a batch of 2; fused mode)."""
     cfg = synth.small_config(1 << 14, 30.0, 2.0, 256, 2048, n_dm=2, n_sig=2, index=51, amp=0.2)
     xs = np.stack([cfg.series(d) for d in range(2)])
